@@ -1,0 +1,265 @@
+"""ctypes binding of oracle/grpic_oracle.c — TEST INFRASTRUCTURE, not the product path.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this module.  It never imports the CUDA package.
+
+The C file is the oracle (plain FP64 statement of PAPER.md Sec. 3.1-3.2); this module
+only marshals numpy arrays.  `sort_reference` is the one piece written in numpy: the
+sort is not in the paper, its key is defined by include/grpic.h (DESIGN.md R-S9).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass, field
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "grpic_oracle.c")
+_LIB = os.path.join(_HERE, "libgrpic_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", _SRC, "-o", _LIB, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Grid(C.Structure):
+    _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("ng", C.c_int32), ("n_iter", C.c_int32),
+                ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double)]
+
+
+_METRIC_NAMES = ["r", "th", "sth", "cth", "Sigma", "Delta", "A", "z", "s1", "s2", "alpha", "beta1",
+                 "hu11", "hu22", "hu33", "hu13", "hd11", "hd22", "hd33", "hd13", "sqrt_h"]
+_DMETRIC_NAMES = ["hu11", "hu22", "hu33", "hu13", "alpha", "beta1"]
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_bp = C.POINTER(C.c_uint8)
+
+
+class _Fields(C.Structure):
+    _fields_ = [(k, _dp) for k in ("D1", "D2", "D3", "B1", "B2", "B3")]
+
+
+class _Current(C.Structure):
+    _fields_ = [(k, _dp) for k in ("J1", "J2", "J3")]
+
+
+class _Particles(C.Structure):
+    _fields_ = [("n", C.c_int64), ("i1", _ip), ("i2", _ip), ("dx1", _dp), ("dx2", _dp),
+                ("u1", _dp), ("u2", _dp), ("u3", _dp), ("phi", _dp),
+                ("i1_prev", _ip), ("i2_prev", _ip), ("dx1_prev", _dp), ("dx2_prev", _dp),
+                ("weight", _dp), ("tag", _bp),
+                ("q_over_m", C.c_double), ("charge", C.c_double), ("massive", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+@dataclass
+class Grid:
+    n1: int
+    n2: int
+    a: float
+    r_min: float
+    r_max: float
+    ng: int = 2
+    n_iter: int = 10
+    small_angle: float = 1e-5
+
+    def c(self) -> _Grid:
+        return _Grid(self.n1, self.n2, self.ng, self.n_iter, self.a, self.r_min, self.r_max, self.small_angle)
+
+    @property
+    def shape(self):
+        return (self.n1 + 2 * self.ng, self.n2 + 2 * self.ng)
+
+
+def _f64(x):
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _ptr(a, t):
+    return a.ctypes.data_as(t)
+
+
+@dataclass
+class Particles:
+    """FP64 SoA particle columns (same columns as include/grpic.h)."""
+    i1: np.ndarray
+    i2: np.ndarray
+    dx1: np.ndarray
+    dx2: np.ndarray
+    u1: np.ndarray
+    u2: np.ndarray
+    u3: np.ndarray
+    weight: np.ndarray
+    tag: np.ndarray
+    phi: np.ndarray | None = None
+    i1_prev: np.ndarray = field(default=None)
+    i2_prev: np.ndarray = field(default=None)
+    dx1_prev: np.ndarray = field(default=None)
+    dx2_prev: np.ndarray = field(default=None)
+    q_over_m: float = 0.0
+    charge: float = 0.0
+    massive: int = 1
+
+    def __post_init__(self):
+        for k in ("i1", "i2"):
+            setattr(self, k, np.ascontiguousarray(getattr(self, k), dtype=np.int32).copy())
+        for k in ("dx1", "dx2", "u1", "u2", "u3", "weight"):
+            setattr(self, k, _f64(getattr(self, k)).copy())
+        self.tag = np.ascontiguousarray(self.tag, dtype=np.uint8).copy()
+        if self.phi is not None:
+            self.phi = _f64(self.phi).copy()
+        n = self.i1.size
+        self.i1_prev = np.zeros(n, np.int32) if self.i1_prev is None else np.ascontiguousarray(self.i1_prev, np.int32).copy()
+        self.i2_prev = np.zeros(n, np.int32) if self.i2_prev is None else np.ascontiguousarray(self.i2_prev, np.int32).copy()
+        self.dx1_prev = np.zeros(n) if self.dx1_prev is None else _f64(self.dx1_prev).copy()
+        self.dx2_prev = np.zeros(n) if self.dx2_prev is None else _f64(self.dx2_prev).copy()
+
+    @property
+    def n(self):
+        return self.i1.size
+
+    def copy(self) -> "Particles":
+        return Particles(**{k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in self.__dict__.items()})
+
+    def c(self) -> _Particles:
+        return _Particles(self.n, _ptr(self.i1, _ip), _ptr(self.i2, _ip), _ptr(self.dx1, _dp), _ptr(self.dx2, _dp),
+                          _ptr(self.u1, _dp), _ptr(self.u2, _dp), _ptr(self.u3, _dp),
+                          _ptr(self.phi, _dp) if self.phi is not None else None,
+                          _ptr(self.i1_prev, _ip), _ptr(self.i2_prev, _ip), _ptr(self.dx1_prev, _dp),
+                          _ptr(self.dx2_prev, _dp), _ptr(self.weight, _dp), _ptr(self.tag, _bp),
+                          float(self.q_over_m), float(self.charge), int(self.massive))
+
+
+def _fields_c(fields):
+    arrs = [_f64(fields[k]) for k in ("D1", "D2", "D3", "B1", "B2", "B3")]
+    return _Fields(*[_ptr(a, _dp) for a in arrs]), arrs
+
+
+def metric(g: Grid, x1, x2, derivs: bool = True):
+    """All S1 quantities (and S2 derivatives) at code coordinates (x1, x2)."""
+    x1 = _f64(np.atleast_1d(x1)); x2 = _f64(np.atleast_1d(x2))
+    n = x1.size
+    m = np.zeros((n, len(_METRIC_NAMES)))
+    d = np.zeros((n, len(_DMETRIC_NAMES), 2))
+    gc = g.c()
+    lib().orc_metric_many(C.byref(gc), C.c_int64(n), _ptr(x1, _dp), _ptr(x2, _dp), _ptr(m, _dp),
+                          _ptr(d, _dp) if derivs else None)
+    out = {k: m[:, j].copy() for j, k in enumerate(_METRIC_NAMES)}
+    if derivs:
+        for j, k in enumerate(_DMETRIC_NAMES):
+            out["d1_" + k] = d[:, j, 0].copy()
+            out["d2_" + k] = d[:, j, 1].copy()
+    return out
+
+
+def _vec3(fn, g, x1, x2, v):
+    gc = g.c()
+    out = np.zeros(3)
+    m = (C.c_double * len(_METRIC_NAMES))()
+    lib().orc_metric(C.byref(gc), C.c_double(x1), C.c_double(x2), m)
+    vin = _f64(v)
+    getattr(lib(), fn)(m, _ptr(vin, _dp), _ptr(out, _dp))
+    return out
+
+
+def cntrv_to_tetrad(g, x1, x2, v): return _vec3("orc_cntrv_to_tetrad", g, x1, x2, v)
+def cov_to_tetrad(g, x1, x2, v): return _vec3("orc_cov_to_tetrad", g, x1, x2, v)
+def tetrad_to_cov(g, x1, x2, v): return _vec3("orc_tetrad_to_cov", g, x1, x2, v)
+def tetrad_to_cntrv(g, x1, x2, v): return _vec3("orc_tetrad_to_cntrv", g, x1, x2, v)
+
+
+def interp(g: Grid, fields, i1, i2, dx1, dx2):
+    fc, keep = _fields_c(fields)
+    i1 = np.ascontiguousarray(i1, np.int32); i2 = np.ascontiguousarray(i2, np.int32)
+    dx1 = _f64(dx1); dx2 = _f64(dx2)
+    n = i1.size
+    D = np.zeros((n, 3)); B = np.zeros((n, 3))
+    gc = g.c()
+    lib().orc_interp_many(C.byref(gc), C.byref(fc), C.c_int64(n), _ptr(i1, _ip), _ptr(i2, _ip),
+                          _ptr(dx1, _dp), _ptr(dx2, _dp), _ptr(D, _dp), _ptr(B, _dp))
+    return D, B
+
+
+def push(g: Grid, p: Particles, fields, dt: float):
+    """In-place step 1-11 + BCs on `p`.  Returns (alive, absorbed_in, absorbed_out)."""
+    gc = g.c(); pc = p.c()
+    cnt = (C.c_int64 * 3)()
+    if fields is None:
+        assert p.q_over_m == 0.0 or not p.massive, "charged particles need fields"
+        lib().orc_push(C.byref(gc), C.byref(pc), None, C.c_double(dt), cnt)
+    else:
+        fc, keep = _fields_c(fields)
+        lib().orc_push(C.byref(gc), C.byref(pc), C.byref(fc), C.c_double(dt), cnt)
+    return tuple(int(x) for x in cnt)
+
+
+def push_given_fields(g: Grid, p: Particles, Dp, Bp, dt: float):
+    """Same update with contravariant D,B at each particle supplied ([n,3])."""
+    gc = g.c(); pc = p.c()
+    Dp = _f64(Dp).reshape(p.n, 3); Bp = _f64(Bp).reshape(p.n, 3)
+    lib().orc_push_given_fields(C.byref(gc), C.byref(pc), _ptr(Dp, _dp), _ptr(Bp, _dp), C.c_double(dt))
+
+
+def deposit(g: Grid, p: Particles, dt: float, J=None):
+    """Accumulate into J = dict(J1,J2,J3) (created zeroed if None). Returns (J, n_overstep)."""
+    if J is None:
+        J = {k: np.zeros(g.shape) for k in ("J1", "J2", "J3")}
+    for k in ("J1", "J2", "J3"):
+        assert J[k].dtype == np.float64 and J[k].flags.c_contiguous and J[k].shape == g.shape
+    jc = _Current(*[_ptr(J[k], _dp) for k in ("J1", "J2", "J3")])
+    gc = g.c(); pc = p.c()
+    over = C.c_int64(0)
+    lib().orc_deposit(C.byref(gc), C.byref(pc), C.c_double(dt), C.byref(jc), C.byref(over))
+    return J, int(over.value)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int):
+    lib().orc_set_num_threads(C.c_int(n))
+
+
+# ----------------------------------------------------------------------------------------------
+# Sort reference (not in the paper; key defined in include/grpic.h, DESIGN.md R-S9).
+# ----------------------------------------------------------------------------------------------
+def sort_key(g: Grid, i1, i2, tag, tile: int):
+    """Tile-major cell key; dead particles get the key one past the last cell."""
+    i1 = np.asarray(i1, np.int64); i2 = np.asarray(i2, np.int64)
+    nt2 = (g.n2 + tile - 1) // tile
+    nt1 = (g.n1 + tile - 1) // tile
+    t1, l1 = i1 // tile, i1 % tile
+    t2, l2 = i2 // tile, i2 % tile
+    key = ((t1 * nt2 + t2) * tile + l1) * tile + l2
+    dead_key = nt1 * nt2 * tile * tile
+    return np.where(np.asarray(tag) != 0, key, dead_key), dead_key
+
+
+def sort_reference(g: Grid, p: Particles, tile: int):
+    """Stable sort of all columns by sort_key. Returns (sorted copy, permutation, keys_sorted)."""
+    key, _ = sort_key(g, p.i1, p.i2, p.tag, tile)
+    perm = np.argsort(key, kind="stable")
+    q = p.copy()
+    for k, v in p.__dict__.items():
+        if isinstance(v, np.ndarray):
+            setattr(q, k, v[perm].copy())
+    return q, perm, key[perm]
