@@ -1,0 +1,159 @@
+/*
+ * grpic.h — C ABI of the B200-native per-particle GRPIC hot path.
+ *
+ * What is behind it: the per-particle step of the general-relativistic particle-in-cell
+ * method of arxiv/paper_2511_17701 ("Entity II: General Relativistic Module") on a 2D
+ * axisymmetric (r, theta) Kerr-Schild grid, as hand-written sm_100a CUDA kernels.
+ * "P:n" below = line n of the paper text; "R-Sk" = reading k of DESIGN.md.
+ *
+ * Two builds of one source export the SAME symbols:
+ *     libgrpic_f32.so   grpic_real = float
+ *     libgrpic_f64.so   grpic_real = double      (compile consumers with -DGRPIC_F64)
+ * grpic_real_bytes() tells which one was loaded.
+ *
+ * Conventions
+ *   - Every pointer inside grpic_particles / grpic_fields / grpic_current is CALLER-OWNED DEVICE
+ *     memory (cudaMalloc'ed, or a torch CUDA tensor's data_ptr).  The *_host entry point is the one
+ *     exception and says so.  The structs themselves live in host memory and are read during the call.
+ *   - The library owns only its context (constants, counters, sort scratch, tile table).
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default
+ *     stream) and return without synchronising, except grpic_counters, grpic_sort's first scratch
+ *     allocation and grpic_step_host.
+ *   - Return value: GRPIC_OK (0) or a negative grpic_status; grpic_last_error(ctx) gives the text.
+ *     Nothing aborts or throws.  There is no CPU fallback: without a CUDA device every compute
+ *     call returns GRPIC_ECUDA.
+ *   - Grid arrays (fields, currents): shape [n1 + 2*nghost][n2 + 2*nghost], i2 fastest, element
+ *     (i1, i2) of the physical mesh at [(i1 + nghost)*(n2 + 2*nghost) + (i2 + nghost)].
+ *     Yee locations (Eq. 40-41):
+ *         D1(i+1/2, j)  D2(i, j+1/2)  D3(i, j)      B1(i, j+1/2)  B2(i+1/2, j)  B3(i+1/2, j+1/2)
+ *     J^i sits where D^i sits.  Components are contravariant, code basis, code units.
+ *     Ghost zones of the fields must be filled by the caller; the path reads one ghost
+ *     layer.  Ghost zones of J are written raw (folding them back is field-side work).
+ *   - Code coordinates: x1 in [0, n1) is radial with r = r_min * exp(x1 * ln(r_max/r_min)/n1)
+ *     (App. A.3 with r0 = 0), x2 in [0, n2) is polar with theta = x2 * pi/n2; a position
+ *     is (cell index i, displacement dx in [0,1)) per axis.  r_g = M = 1.
+ */
+#ifndef GRPIC_H_
+#define GRPIC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#ifdef GRPIC_F64
+typedef double grpic_real;
+#else
+typedef float grpic_real;
+#endif
+
+typedef enum {
+  GRPIC_OK = 0,
+  GRPIC_EINVAL = -1, /* bad argument (NULL pointer, n < 0, nghost < 1, ...)        */
+  GRPIC_ENOMEM = -2, /* device or host allocation failed                           */
+  GRPIC_ECUDA = -3,  /* CUDA runtime error or no device (text in grpic_last_error) */
+  GRPIC_ESTATE = -4  /* call out of order (deposit before any push, ...)           */
+} grpic_status;
+
+typedef struct grpic_ctx grpic_ctx; /* opaque, library-owned */
+
+/* The mesh: n1 = N_r, n2 = N_theta cells, nghost >= 1 ghost layers on every side. */
+typedef struct {
+  int32_t n1, n2, nghost;
+  int32_t r_map; /* 1 = logarithmic r (App. A.3, r0 = 0, h0 = 0). Only 1 is built. */
+} grpic_grid;
+
+/* One species, structure-of-arrays.
+ * Columns of length >= n; slots with tag == 0 are dead and ignored by every call.
+ * 16-byte alignment of every column is required (torch / cudaMalloc give 256). */
+typedef struct {
+  int64_t n;                   /* slots in use (alive + dead)                                   */
+  int32_t *i1, *i2;            /* cell index                                     in/out         */
+  grpic_real *dx1, *dx2;       /* displacement in [0,1)                          in/out         */
+  grpic_real *u1, *u2, *u3;    /* covariant four-velocity, code basis            in/out         */
+  grpic_real *phi;             /* out-of-plane angle (Eq. 30); may be NULL       in/out         */
+  int32_t *i1_prev, *i2_prev;  /* position before the push: written by push,     read by deposit */
+  grpic_real *dx1_prev, *dx2_prev;
+  const grpic_real *weight;    /* macro-particle weight                          in             */
+  uint8_t *tag;                /* 1 alive, 0 dead                                in/out         */
+  double q_over_m;             /* charge/mass in code units; 0 skips the EM push        */
+  double charge;               /* charge of one unit of weight, multiplies the deposit (Eq. 33) */
+  int32_t massive;             /* 1: gamma = sqrt(1 + h^ij u_i u_j); 0: massless (Eq. 20), no EM push */
+} grpic_particles;
+
+typedef struct { const grpic_real *D1, *D2, *D3, *B1, *B2, *B3; } grpic_fields;
+typedef struct { grpic_real *J1, *J2, *J3; } grpic_current; /* ACCUMULATED into; caller zeroes */
+
+/* sizeof(grpic_real) of the loaded build: 4 or 8. */
+int grpic_real_bytes(void);
+
+/* Create a context for one mesh and one Kerr spin a (|a| < 1... <= 1), radial extent [r_min, r_max]
+ * in units of r_g (north_star: grpic_create(grid, a, r_min, r_max); metric of App. A.3).
+ * Defaults: n_iter = 10, small_angle = 1e-5 (SMALL_ANGLE_GR).
+ * Errors: EINVAL (NULL, n1/n2 < 1, nghost < 1, r_map != 1, r_min <= 0 or >= r_max), ECUDA, ENOMEM. */
+int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, grpic_ctx** out);
+int grpic_destroy(grpic_ctx* ctx);
+
+/* "n_iter": fixed iteration count of the two midpoint integrators, 1..64.
+ * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernel after a grpic_sort;
+ *              0 forces the direct kernel (global gathers and atomics). */
+int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t value);
+/* "small_angle": theta used in any metric evaluation is clamped to [eps, pi - eps] (R-S9). */
+int grpic_set_real(grpic_ctx* ctx, const char* key, double value);
+
+/* Steps 1-11 of Sec. 3.1 for every alive particle, then the particle boundary
+ * conditions: save previous position; interpolate D, B (R-S4); tetrad-frame Boris half
+ * push (Eq. 19, R-S5); geodesic momentum push (Eq. 26-27); second half push; geodesic coordinate
+ * push (Eq. 28-29); phi (Eq. 30); renormalise (i, dx); reflect at the axes; tag = 0 for i1 < 0
+ * (inside the horizon) or i1 >= n1.  `fields` may be NULL iff q_over_m == 0 or massive == 0.
+ * Remembers dt for grpic_deposit.  Errors: EINVAL, ECUDA. */
+int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, double dt,
+                      void* cuda_stream);
+
+/* Charge-conserving conformal current deposit (Sec. 3.2, Eq. 32-36; scheme R-S10) from
+ * (i*_prev, dx*_prev) to (i*, dx*) of every alive particle, with the dt of the last push on this
+ * context.  J += ; a no-op if charge == 0.  A particle that moved more than one cell along an axis
+ * is skipped and counted (n_overstep).  Errors: EINVAL, ESTATE (no push yet), ECUDA. */
+int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, void* cuda_stream);
+
+/* Fused grpic_interp_push + grpic_deposit in one kernel (previous position stays in registers but is
+ * still written, so that grpic_deposit / diagnostics see it).  Same results as the two calls up to
+ * the order of the J additions.  J may be NULL iff charge == 0. */
+int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, grpic_current* J,
+               double dt, void* cuda_stream);
+
+/* Counting sort of all columns by tile-major cell key (not in the paper; north_star names it; R-S9):
+ *     key = ((i1/T * ceil(n2/T) + i2/T) * T + i1%T) * T + i2%T,  T = grpic_tile_size(),
+ * dead particles after all alive ones.  In place from the caller's view (library scratch inside).
+ * Any order within one key is a correct result.  Builds the tile table that grpic_step's
+ * shared-memory path uses for this species (keyed by the address of p->i1).
+ * Errors: EINVAL, ENOMEM, ECUDA. */
+int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* cuda_stream);
+int grpic_tile_size(void);
+
+/* Counters of the most recent push/step (alive after it, absorbed inside, absorbed outside) and
+ * of the most recent deposit/step (n_overstep).  Synchronises `cuda_stream`. Any pointer may be NULL. */
+int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_absorbed_in, int64_t* n_absorbed_out,
+                   int64_t* n_overstep, void* cuda_stream);
+
+/* Number of particle updates (alive particles pushed) by all push/step calls since grpic_create:
+ * the numerator of the throughput metric.  Synchronises `cuda_stream`. */
+int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* cuda_stream);
+
+/* End-to-end convenience: every pointer in p, fields and J is HOST memory (pinned or pageable).
+ * Copies fields and particle columns to library-owned device buffers in chunks, runs the fused step
+ * chunk by chunk (copies overlapped with compute on two streams), accumulates J on the device and
+ * copies the particle columns and J back; J_host += .  Synchronous.  Bytes moved are reported through
+ * h2d_bytes / d2h_bytes (may be NULL).  Errors as grpic_step, plus ENOMEM. */
+int grpic_step_host(grpic_ctx* ctx, grpic_particles* p_host, const grpic_fields* fields_host,
+                    grpic_current* J_host, double dt, int64_t* h2d_bytes, int64_t* d2h_bytes);
+
+/* Text of the last error on this context (or of the last failed grpic_create if ctx == NULL).
+ * Owned by the library, valid until the next call. */
+const char* grpic_last_error(grpic_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRPIC_H_ */

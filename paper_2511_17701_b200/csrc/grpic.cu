@@ -1,0 +1,567 @@
+// grpic.cu — host side of the C ABI declared in include/grpic.h: argument checks, context,
+// launches.  One source, two builds (-DGRPIC_F64 selects grpic_real = double).
+// There is no CPU fallback anywhere in this file: every compute entry point launches CUDA kernels
+// or returns an error.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/grpic.h"
+#include "grpic_kernels.cuh"
+#include "grpic_tiled.cuh"
+
+using namespace grpic;
+typedef grpic_real real;
+
+namespace {
+
+std::string g_create_error;
+
+struct SortState {          // tile table of one species (keyed by the address of its i1 column)
+  int64_t n_at_sort = 0;    // p->n when the table was built
+  WorkItem* items = nullptr;
+  uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time
+  uint32_t max_items = 0;
+};
+
+}  // namespace
+
+struct grpic_ctx {
+  grpic_grid grid;
+  double a, r_min, r_max, small_angle;
+  int n_iter, tile_path;
+  double last_dt;
+  bool have_dt;
+  unsigned long long* d_counters;   // 5: four of the last call + cumulative updates
+  std::string err;
+  int device;
+  // sort scratch
+  uint32_t *d_keys, *d_dest, *d_hist, *d_block_sums, *d_tile_items;
+  int64_t cap_particles;
+  void* d_scratch;
+  size_t scratch_bytes;
+  std::map<const void*, SortState> sorted;
+  // TMA
+  TmaEncoder tma;
+  // grpic_step_host buffers
+  void* h_dev[16];
+  size_t h_cap;
+  void* h_fields;
+  size_t h_fields_bytes;
+  cudaStream_t h_streams[2];
+  bool h_streams_ok;
+};
+
+namespace {
+
+int fail(grpic_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+int cuda_fail(grpic_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, GRPIC_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);  \
+  } while (0)
+
+Consts<real> make_consts(const grpic_ctx* c) {
+  Consts<real> g;
+  g.n1 = c->grid.n1; g.n2 = c->grid.n2; g.ng = c->grid.nghost; g.n_iter = c->n_iter;
+  g.ld = c->grid.n2 + 2 * c->grid.nghost;
+  g.pad_ = 0;
+  const double dxi = std::log(c->r_max / c->r_min) / c->grid.n1;
+  const double deta = M_PI / c->grid.n2;
+  g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
+  g.log_rmin = (real)std::log(c->r_min);
+  g.dxi = (real)dxi; g.deta = (real)deta;
+  g.half_dxi = (real)(0.5 * dxi); g.half_deta = (real)(0.5 * deta);
+  g.inv_deta2 = (real)(1.0 / (deta * deta));
+  g.th_min = (real)c->small_angle;
+  g.th_max = (real)(M_PI - c->small_angle);
+  return g;
+}
+
+PPtrs<real> make_pptrs(const grpic_particles* p) {
+  PPtrs<real> P;
+  P.n = p->n;
+  P.i1 = p->i1; P.i2 = p->i2; P.dx1 = p->dx1; P.dx2 = p->dx2;
+  P.u1 = p->u1; P.u2 = p->u2; P.u3 = p->u3; P.phi = p->phi;
+  P.i1p = p->i1_prev; P.i2p = p->i2_prev; P.dx1p = p->dx1_prev; P.dx2p = p->dx2_prev;
+  P.w = p->weight; P.tag = p->tag;
+  return P;
+}
+
+int check_particles(grpic_ctx* ctx, const grpic_particles* p, bool need_prev) {
+  if (!p) return fail(ctx, GRPIC_EINVAL, "particles == NULL");
+  if (p->n < 0) return fail(ctx, GRPIC_EINVAL, "particles.n < 0");
+  if (p->n > 0xfffffff0ll) return fail(ctx, GRPIC_EINVAL, "particles.n exceeds 2^32 - 16");
+  if (p->n == 0) return GRPIC_OK;
+  if (!p->i1 || !p->i2 || !p->dx1 || !p->dx2 || !p->u1 || !p->u2 || !p->u3 || !p->weight || !p->tag)
+    return fail(ctx, GRPIC_EINVAL, "a required particle column is NULL");
+  if (need_prev && (!p->i1_prev || !p->i2_prev || !p->dx1_prev || !p->dx2_prev))
+    return fail(ctx, GRPIC_EINVAL, "a *_prev particle column is NULL");
+  return GRPIC_OK;
+}
+
+SpeciesConst make_species(const grpic_particles* p, double dt, bool deposit) {
+  SpeciesConst sc;
+  sc.q_over_m = p->q_over_m; sc.charge = p->charge; sc.dt = dt;
+  sc.massive = p->massive ? 1 : 0;
+  sc.em = (p->q_over_m != 0.0 && p->massive) ? 1 : 0;
+  sc.has_phi = p->phi ? 1 : 0;
+  sc.do_deposit = (deposit && p->charge != 0.0) ? 1 : 0;
+  return sc;
+}
+
+int check_fields(grpic_ctx* ctx, const grpic_fields* f, const SpeciesConst& sc, FPtrs<real>& F) {
+  for (int k = 0; k < 6; ++k) F.f[k] = nullptr;
+  if (!sc.em) return GRPIC_OK;
+  if (!f) return fail(ctx, GRPIC_EINVAL, "fields == NULL for a charged massive species");
+  const real* a[6] = {f->D1, f->D2, f->D3, f->B1, f->B2, f->B3};
+  for (int k = 0; k < 6; ++k) {
+    if (!a[k]) return fail(ctx, GRPIC_EINVAL, "a field component pointer is NULL");
+    F.f[k] = a[k];
+  }
+  return GRPIC_OK;
+}
+
+int check_current(grpic_ctx* ctx, const grpic_current* J, const SpeciesConst& sc, JPtrs<real>& Jp) {
+  for (int k = 0; k < 3; ++k) Jp.j[k] = nullptr;
+  if (!sc.do_deposit) return GRPIC_OK;
+  if (!J || !J->J1 || !J->J2 || !J->J3) return fail(ctx, GRPIC_EINVAL, "current pointers are NULL for a charged species");
+  Jp.j[0] = J->J1; Jp.j[1] = J->J2; Jp.j[2] = J->J3;
+  return GRPIC_OK;
+}
+
+inline unsigned grid_for(int64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
+
+int scan_exclusive(grpic_ctx* ctx, uint32_t* d, uint32_t n, cudaStream_t st) {
+  const uint32_t nb = (n + kScanTile - 1) / kScanTile;
+  k_scan_local<<<nb, kScanBlock, 0, st>>>(d, n, ctx->d_block_sums);
+  k_scan_sums<<<1, kScanBlock, 0, st>>>(ctx->d_block_sums, nb);
+  k_scan_add<<<nb, kScanBlock, 0, st>>>(d, n, ctx->d_block_sums);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+SortGeom sort_geom(const grpic_ctx* c) {
+  SortGeom s;
+  s.n1 = c->grid.n1; s.n2 = c->grid.n2;
+  s.nt1 = (c->grid.n1 + kTile - 1) / kTile;
+  s.nt2 = (c->grid.n2 + kTile - 1) / kTile;
+  s.n_keys = (uint32_t)s.nt1 * s.nt2 * kTile * kTile + 1u;
+  return s;
+}
+
+void free_sort_state(SortState& s) {
+  if (s.items) cudaFree(s.items);
+  if (s.d_n_items) cudaFree(s.d_n_items);
+  s = SortState();
+}
+
+}  // namespace
+
+extern "C" {
+
+int grpic_real_bytes(void) { return (int)sizeof(real); }
+int grpic_tile_size(void) { return kTile; }
+
+const char* grpic_last_error(grpic_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, grpic_ctx** out) {
+  grpic_ctx* ctx = nullptr;
+  if (!grid || !out) return fail(nullptr, GRPIC_EINVAL, "grid or out is NULL");
+  *out = nullptr;
+  if (grid->n1 < 1 || grid->n2 < 1) return fail(nullptr, GRPIC_EINVAL, "n1, n2 must be >= 1");
+  if (grid->nghost < 1) return fail(nullptr, GRPIC_EINVAL, "nghost must be >= 1 (the gather reads one ghost layer)");
+  if (grid->r_map != 1) return fail(nullptr, GRPIC_EINVAL, "only r_map = 1 (logarithmic r, App. A.3) is built");
+  if (!(r_min > 0.0) || !(r_max > r_min)) return fail(nullptr, GRPIC_EINVAL, "need 0 < r_min < r_max");
+  if (!(std::fabs(a) <= 1.0)) return fail(nullptr, GRPIC_EINVAL, "need |a| <= 1");
+  if ((int64_t)(grid->n1 + 2 * grid->nghost) * (grid->n2 + 2 * grid->nghost) > 0x7fffffffll)
+    return fail(nullptr, GRPIC_EINVAL, "grid too large");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev < 1)
+    return fail(nullptr, GRPIC_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
+  ctx = new (std::nothrow) grpic_ctx();
+  if (!ctx) return fail(nullptr, GRPIC_ENOMEM, "host allocation failed");
+  ctx->grid = *grid;
+  ctx->a = a; ctx->r_min = r_min; ctx->r_max = r_max;
+  ctx->small_angle = 1e-5;                                  // SMALL_ANGLE_GR
+  ctx->n_iter = 10;
+  ctx->tile_path = 1;
+  ctx->have_dt = false; ctx->last_dt = 0.0;
+  ctx->d_counters = nullptr;
+  ctx->d_keys = ctx->d_dest = ctx->d_hist = ctx->d_block_sums = ctx->d_tile_items = nullptr;
+  ctx->cap_particles = 0;
+  ctx->d_scratch = nullptr; ctx->scratch_bytes = 0;
+  for (auto& q : ctx->h_dev) q = nullptr;
+  ctx->h_cap = 0; ctx->h_fields = nullptr; ctx->h_fields_bytes = 0; ctx->h_streams_ok = false;
+  cudaGetDevice(&ctx->device);
+  e = cudaMalloc(&ctx->d_counters, 8 * sizeof(unsigned long long));
+  if (e != cudaSuccess) {
+    std::string m = std::string("cudaMalloc(counters): ") + cudaGetErrorString(e);
+    delete ctx;
+    return fail(nullptr, GRPIC_ECUDA, m);
+  }
+  cudaMemset(ctx->d_counters, 0, 8 * sizeof(unsigned long long));
+  ctx->tma.init();
+  *out = ctx;
+  return GRPIC_OK;
+}
+
+int grpic_destroy(grpic_ctx* ctx) {
+  if (!ctx) return GRPIC_OK;
+  cudaDeviceSynchronize();
+  for (auto& kv : ctx->sorted) free_sort_state(kv.second);
+  cudaFree(ctx->d_counters);
+  cudaFree(ctx->d_keys); cudaFree(ctx->d_dest); cudaFree(ctx->d_hist);
+  cudaFree(ctx->d_block_sums); cudaFree(ctx->d_tile_items);
+  cudaFree(ctx->d_scratch);
+  for (auto q : ctx->h_dev) cudaFree(q);
+  cudaFree(ctx->h_fields);
+  if (ctx->h_streams_ok) { cudaStreamDestroy(ctx->h_streams[0]); cudaStreamDestroy(ctx->h_streams[1]); }
+  delete ctx;
+  return GRPIC_OK;
+}
+
+int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t v) {
+  if (!ctx || !key) return fail(ctx, GRPIC_EINVAL, "ctx or key is NULL");
+  if (!std::strcmp(key, "n_iter")) {
+    if (v < 1 || v > 64) return fail(ctx, GRPIC_EINVAL, "n_iter must be in 1..64");
+    ctx->n_iter = (int)v;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "tile_path")) {
+    ctx->tile_path = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  return fail(ctx, GRPIC_EINVAL, std::string("unknown integer key: ") + key);
+}
+
+int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
+  if (!ctx || !key) return fail(ctx, GRPIC_EINVAL, "ctx or key is NULL");
+  if (!std::strcmp(key, "small_angle")) {
+    if (!(v >= 0.0 && v < 1.0)) return fail(ctx, GRPIC_EINVAL, "small_angle must be in [0, 1)");
+    ctx->small_angle = v;
+    return GRPIC_OK;
+  }
+  return fail(ctx, GRPIC_EINVAL, std::string("unknown real key: ") + key);
+}
+
+int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, double dt, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, p, true);
+  if (rc) return rc;
+  if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
+  const SpeciesConst sc = make_species(p, dt, false);
+  FPtrs<real> F;
+  if ((rc = check_fields(ctx, fields, sc, F))) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  ctx->last_dt = dt; ctx->have_dt = true;
+  CK(cudaMemsetAsync(ctx->d_counters, 0, 3 * sizeof(unsigned long long), st));
+  if (p->n == 0) return GRPIC_OK;
+  JPtrs<real> J{{nullptr, nullptr, nullptr}};
+  k_push_or_step<real, false><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), F, J, sc,
+                                                                 ctx->d_counters);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, p, true);
+  if (rc) return rc;
+  if (!ctx->have_dt) return fail(ctx, GRPIC_ESTATE, "grpic_deposit before any grpic_interp_push on this context");
+  const SpeciesConst sc = make_species(p, ctx->last_dt, true);
+  JPtrs<real> Jp;
+  if ((rc = check_current(ctx, J, sc, Jp))) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  CK(cudaMemsetAsync(ctx->d_counters + 3, 0, sizeof(unsigned long long), st));
+  if (p->n == 0 || !sc.do_deposit) return GRPIC_OK;
+  k_deposit<real><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, grpic_current* J, double dt,
+               void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, p, true);
+  if (rc) return rc;
+  if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
+  const SpeciesConst sc = make_species(p, dt, true);
+  FPtrs<real> F;
+  JPtrs<real> Jp;
+  if ((rc = check_fields(ctx, fields, sc, F))) return rc;
+  if ((rc = check_current(ctx, J, sc, Jp))) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  ctx->last_dt = dt; ctx->have_dt = true;
+  CK(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), st));
+  if (p->n == 0) return GRPIC_OK;
+  const Consts<real> g = make_consts(ctx);
+  const PPtrs<real> P = make_pptrs(p);
+
+  auto it = ctx->sorted.find((const void*)p->i1);
+  const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_at_sort <= p->n && sc.em &&
+                     sc.do_deposit;
+  if (!tiled) {
+    k_push_or_step<real, true><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    CK(cudaGetLastError());
+    return GRPIC_OK;
+  }
+  const SortState& ss = it->second;
+  std::string terr;
+  if (!launch_step_tiled<real>(ctx->tma, g, P, F, Jp, sc, ctx->d_counters, ss.items, ss.d_n_items, ss.max_items,
+                               ss.n_at_sort, st, terr))
+    return fail(ctx, GRPIC_ECUDA, terr);
+  return GRPIC_OK;
+}
+
+int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, p, true);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = p->n;
+  if (n == 0) return GRPIC_OK;
+  const SortGeom sg = sort_geom(ctx);
+  const uint32_t n_tiles = (uint32_t)sg.nt1 * sg.nt2;
+  // scratch (grown on demand; growing synchronises)
+  const size_t col = ((size_t)n * sizeof(real) + 255) / 256 * 256;
+  const size_t col4 = ((size_t)n * 4 + 255) / 256 * 256;
+  const size_t col1 = ((size_t)n + 255) / 256 * 256;
+  const size_t need = 9 * col + 4 * col4 + col1;
+  if (ctx->cap_particles < n) {
+    CK(cudaStreamSynchronize(st));
+    cudaFree(ctx->d_keys); cudaFree(ctx->d_dest);
+    ctx->d_keys = ctx->d_dest = nullptr; ctx->cap_particles = 0;
+    if (cudaMalloc(&ctx->d_keys, (size_t)n * 4) != cudaSuccess || cudaMalloc(&ctx->d_dest, (size_t)n * 4) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ctx, GRPIC_ENOMEM, "sort scratch (keys) allocation failed");
+    }
+    ctx->cap_particles = n;
+  }
+  if (ctx->scratch_bytes < need) {
+    CK(cudaStreamSynchronize(st));
+    cudaFree(ctx->d_scratch); ctx->d_scratch = nullptr; ctx->scratch_bytes = 0;
+    if (cudaMalloc(&ctx->d_scratch, need) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ctx, GRPIC_ENOMEM, "sort scratch (columns) allocation failed");
+    }
+    ctx->scratch_bytes = need;
+  }
+  if (!ctx->d_hist) {
+    const uint32_t nb = (sg.n_keys + 1 + kScanTile - 1) / kScanTile + 1;
+    if (cudaMalloc(&ctx->d_hist, ((size_t)sg.n_keys + 1) * 4) != cudaSuccess ||
+        cudaMalloc(&ctx->d_block_sums, (size_t)(nb + 1024) * 4) != cudaSuccess ||
+        cudaMalloc(&ctx->d_tile_items, ((size_t)n_tiles + 1) * 4) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ctx, GRPIC_ENOMEM, "sort scratch (histogram) allocation failed");
+    }
+  }
+  // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks; 4. scatter all columns; 5. copy back
+  CK(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)sg.n_keys + 1) * 4, st));
+  k_sort_hist<<<grid_for(n), kBlock, 0, st>>>(sg, n, p->i1, p->i2, p->tag, ctx->d_keys, ctx->d_hist);
+  if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
+
+  // tile table from the offsets (before the cursor copy is consumed)
+  SortState& ss = ctx->sorted[(const void*)p->i1];
+  const uint32_t max_items = n_tiles + (uint32_t)((n + kChunk - 1) / kChunk);
+  if (ss.max_items < max_items) {
+    CK(cudaStreamSynchronize(st));
+    free_sort_state(ss);
+    if (cudaMalloc(&ss.items, (size_t)max_items * sizeof(WorkItem)) != cudaSuccess ||
+        cudaMalloc(&ss.d_n_items, 2 * sizeof(uint32_t)) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->sorted.erase((const void*)p->i1);
+      return fail(ctx, GRPIC_ENOMEM, "tile table allocation failed");
+    }
+    ss.max_items = max_items;
+  }
+  ss.n_at_sort = n;
+  k_items_count<<<(n_tiles + 255) / 256, 256, 0, st>>>(ctx->d_hist, n_tiles, ctx->d_tile_items);
+  if ((rc = scan_exclusive(ctx, ctx->d_tile_items, n_tiles, st))) return rc;
+  k_items_fill<<<(n_tiles + 255) / 256, 256, 0, st>>>(ctx->d_hist, n_tiles, ctx->d_tile_items, ss.items,
+                                                      ss.d_n_items, ss.d_n_items + 1);
+
+  k_sort_rank<<<grid_for(n), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
+
+  char* s = (char*)ctx->d_scratch;
+  PPtrs<real> in = make_pptrs(p), out;
+  out.n = n;
+  out.dx1 = (real*)s; s += col; out.dx2 = (real*)s; s += col;
+  out.u1 = (real*)s; s += col; out.u2 = (real*)s; s += col; out.u3 = (real*)s; s += col;
+  out.phi = (real*)s; s += col;
+  out.dx1p = (real*)s; s += col; out.dx2p = (real*)s; s += col;
+  out.w = (const real*)s; s += col;
+  out.i1 = (int32_t*)s; s += col4; out.i2 = (int32_t*)s; s += col4;
+  out.i1p = (int32_t*)s; s += col4; out.i2p = (int32_t*)s; s += col4;
+  out.tag = (uint8_t*)s;
+  k_sort_scatter<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
+  CK(cudaGetLastError());
+  const size_t rb = (size_t)n * sizeof(real), ib = (size_t)n * 4;
+  CK(cudaMemcpyAsync(p->dx1, out.dx1, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->dx2, out.dx2, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->u1, out.u1, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->u2, out.u2, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->u3, out.u3, rb, cudaMemcpyDeviceToDevice, st));
+  if (p->phi) CK(cudaMemcpyAsync(p->phi, out.phi, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->dx1_prev, out.dx1p, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->dx2_prev, out.dx2p, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync((void*)p->weight, out.w, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->i1, out.i1, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->i2, out.i2, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->i1_prev, out.i1p, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->i2_prev, out.i2p, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(p->tag, out.tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
+  return GRPIC_OK;
+}
+
+int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_in, int64_t* n_out, int64_t* n_over, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  unsigned long long h[4];
+  CK(cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CK(cudaStreamSynchronize((cudaStream_t)stream));
+  if (n_alive) *n_alive = (int64_t)h[0];
+  if (n_in) *n_in = (int64_t)h[1];
+  if (n_out) *n_out = (int64_t)h[2];
+  if (n_over) *n_over = (int64_t)h[3];
+  return GRPIC_OK;
+}
+
+int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* stream) {
+  if (!ctx || !n_updates) return fail(ctx, GRPIC_EINVAL, "ctx or n_updates is NULL");
+  unsigned long long h = 0;
+  CK(cudaMemcpyAsync(&h, ctx->d_counters + 4, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CK(cudaStreamSynchronize((cudaStream_t)stream));
+  *n_updates = (int64_t)h;
+  return GRPIC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host-buffer end-to-end step: chunked H2D -> fused step -> D2H on two streams.
+// ------------------------------------------------------------------------------------------------
+int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh, grpic_current* Jh, double dt,
+                    int64_t* h2d_bytes, int64_t* d2h_bytes) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, ph, true);
+  if (rc) return rc;
+  if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
+  const SpeciesConst sc = make_species(ph, dt, true);
+  if (sc.em && (!fh || !fh->D1 || !fh->D2 || !fh->D3 || !fh->B1 || !fh->B2 || !fh->B3))
+    return fail(ctx, GRPIC_EINVAL, "host field pointers are NULL for a charged massive species");
+  if (sc.do_deposit && (!Jh || !Jh->J1 || !Jh->J2 || !Jh->J3))
+    return fail(ctx, GRPIC_EINVAL, "host current pointers are NULL for a charged species");
+  int64_t up = 0, down = 0;
+  const size_t cells = (size_t)(ctx->grid.n1 + 2 * ctx->grid.nghost) * (ctx->grid.n2 + 2 * ctx->grid.nghost);
+  const size_t gbytes = cells * sizeof(real);
+  if (!ctx->h_streams_ok) {
+    CK(cudaStreamCreateWithFlags(&ctx->h_streams[0], cudaStreamNonBlocking));
+    CK(cudaStreamCreateWithFlags(&ctx->h_streams[1], cudaStreamNonBlocking));
+    ctx->h_streams_ok = true;
+  }
+  if (ctx->h_fields_bytes < 9 * gbytes) {
+    cudaFree(ctx->h_fields); ctx->h_fields = nullptr; ctx->h_fields_bytes = 0;
+    if (cudaMalloc(&ctx->h_fields, 9 * gbytes) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ctx, GRPIC_ENOMEM, "device grid buffers allocation failed");
+    }
+    ctx->h_fields_bytes = 9 * gbytes;
+  }
+  const int64_t chunk = 1 << 22;                       // particles per chunk
+  const size_t cb = (size_t)chunk * 8;                 // widest column
+  if (ctx->h_cap < cb) {
+    for (auto& q : ctx->h_dev) { cudaFree(q); q = nullptr; }
+    ctx->h_cap = 0;
+    for (auto& q : ctx->h_dev)
+      if (cudaMalloc(&q, 2 * cb) != cudaSuccess) {      // double-buffered: [0, cb) and [cb, 2cb)
+        cudaGetLastError();
+        return fail(ctx, GRPIC_ENOMEM, "device particle chunk allocation failed");
+      }
+    ctx->h_cap = cb;
+  }
+  cudaStream_t s0 = ctx->h_streams[0];
+  real* dgrid = (real*)ctx->h_fields;
+  FPtrs<real> F;
+  for (int k = 0; k < 6; ++k) F.f[k] = nullptr;
+  if (sc.em) {
+    const real* src[6] = {fh->D1, fh->D2, fh->D3, fh->B1, fh->B2, fh->B3};
+    for (int k = 0; k < 6; ++k) {
+      CK(cudaMemcpyAsync(dgrid + k * cells, src[k], gbytes, cudaMemcpyHostToDevice, s0));
+      F.f[k] = dgrid + k * cells;
+      up += (int64_t)gbytes;
+    }
+  }
+  JPtrs<real> Jp{{nullptr, nullptr, nullptr}};
+  if (sc.do_deposit) {
+    CK(cudaMemsetAsync(dgrid + 6 * cells, 0, 3 * gbytes, s0));
+    for (int k = 0; k < 3; ++k) Jp.j[k] = dgrid + (6 + k) * cells;
+  }
+  CK(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), s0));
+  CK(cudaStreamSynchronize(s0));
+  ctx->last_dt = dt; ctx->have_dt = true;
+  const Consts<real> g = make_consts(ctx);
+  int buf = 0;
+  for (int64_t lo = 0; lo < ph->n; lo += chunk, buf ^= 1) {
+    const int64_t m = (ph->n - lo < chunk) ? ph->n - lo : chunk;
+    cudaStream_t st = ctx->h_streams[buf];
+    char* base[16];
+    for (int k = 0; k < 16; ++k) base[k] = (char*)ctx->h_dev[k] + (size_t)buf * cb;
+    PPtrs<real> P;
+    P.n = m;
+    P.i1 = (int32_t*)base[0]; P.i2 = (int32_t*)base[1];
+    P.dx1 = (real*)base[2]; P.dx2 = (real*)base[3];
+    P.u1 = (real*)base[4]; P.u2 = (real*)base[5]; P.u3 = (real*)base[6];
+    P.phi = ph->phi ? (real*)base[7] : nullptr;
+    P.i1p = (int32_t*)base[8]; P.i2p = (int32_t*)base[9];
+    P.dx1p = (real*)base[10]; P.dx2p = (real*)base[11];
+    P.w = (const real*)base[12]; P.tag = (uint8_t*)base[13];
+    const size_t rb = (size_t)m * sizeof(real), ib = (size_t)m * 4;
+#define UP(dst, src, bytes) do { CK(cudaMemcpyAsync((void*)(dst), (src) + lo, bytes, cudaMemcpyHostToDevice, st)); up += (int64_t)(bytes); } while (0)
+#define DOWN(dst, src, bytes) do { CK(cudaMemcpyAsync((dst) + lo, (src), bytes, cudaMemcpyDeviceToHost, st)); down += (int64_t)(bytes); } while (0)
+    UP(P.i1, ph->i1, ib); UP(P.i2, ph->i2, ib);
+    UP(P.dx1, ph->dx1, rb); UP(P.dx2, ph->dx2, rb);
+    UP(P.u1, ph->u1, rb); UP(P.u2, ph->u2, rb); UP(P.u3, ph->u3, rb);
+    if (P.phi) UP(P.phi, ph->phi, rb);
+    UP(P.w, ph->weight, rb); UP(P.tag, ph->tag, (size_t)m);
+    k_push_or_step<real, true><<<grid_for(m), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    CK(cudaGetLastError());
+    DOWN(ph->i1, P.i1, ib); DOWN(ph->i2, P.i2, ib);
+    DOWN(ph->dx1, P.dx1, rb); DOWN(ph->dx2, P.dx2, rb);
+    DOWN(ph->u1, P.u1, rb); DOWN(ph->u2, P.u2, rb); DOWN(ph->u3, P.u3, rb);
+    if (P.phi) DOWN(ph->phi, P.phi, rb);
+    DOWN(ph->i1_prev, P.i1p, ib); DOWN(ph->i2_prev, P.i2p, ib);
+    DOWN(ph->dx1_prev, P.dx1p, rb); DOWN(ph->dx2_prev, P.dx2p, rb);
+    DOWN(ph->tag, P.tag, (size_t)m);
+#undef UP
+#undef DOWN
+  }
+  CK(cudaStreamSynchronize(ctx->h_streams[0]));
+  CK(cudaStreamSynchronize(ctx->h_streams[1]));
+  if (sc.do_deposit) {
+    std::vector<real> tmp;
+    try { tmp.resize(cells); } catch (...) { return fail(ctx, GRPIC_ENOMEM, "host staging allocation failed"); }
+    real* dst[3] = {Jh->J1, Jh->J2, Jh->J3};
+    for (int k = 0; k < 3; ++k) {
+      CK(cudaMemcpy(tmp.data(), dgrid + (6 + k) * cells, gbytes, cudaMemcpyDeviceToHost));
+      down += (int64_t)gbytes;
+      for (size_t c = 0; c < cells; ++c) dst[k][c] += tmp[c];
+    }
+  }
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = down;
+  return GRPIC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,339 @@
+// grpic_kernels.cuh — the CUDA kernels behind include/grpic.h (sm_100a).
+//
+//   k_push          steps 1-11 + particle BCs, one thread per particle          (grpic_interp_push)
+//   k_deposit       charge-conserving deposit from (prev, current)              (grpic_deposit)
+//   k_step_direct   fused push + deposit, global gathers and global reductions  (grpic_step, unsorted)
+//   k_step_tiled    fused push + deposit over cell-sorted tiles: field stencil of the tile staged
+//                   in shared memory by TMA, J accumulated in shared memory with warp-aggregated
+//                   atomics and flushed once                                    (grpic_step, sorted)
+//   k_sort_*        counting sort by tile-major cell key + tile work-item table (grpic_sort)
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "grpic_device.cuh"
+
+namespace grpic {
+
+constexpr int kTile = 16;                       // cells per tile edge (sort key and shared-memory tile)
+constexpr int kHalo = 3;                        // extra cells around a tile served from shared memory
+constexpr int kWinC = kTile + 2 * kHalo;        // cells per window edge                     (22)
+constexpr int kWinF = kWinC + 2;                // field samples per window edge: c-1 .. c+1 (24)
+constexpr int kWinJ = kWinC + 1;                // J nodes per window edge: c .. c+1         (23)
+constexpr int kChunk = 4096;                    // max particles per work item
+constexpr int kBlock = 256;
+
+template <typename T>
+struct PPtrs {
+  int64_t n;
+  int32_t *i1, *i2;
+  T *dx1, *dx2, *u1, *u2, *u3, *phi;
+  int32_t *i1p, *i2p;
+  T *dx1p, *dx2p;
+  const T* w;
+  uint8_t* tag;
+};
+template <typename T>
+struct FPtrs {
+  const T* f[6];  // D1 D2 D3 B1 B2 B3
+};
+template <typename T>
+struct JPtrs {
+  T* j[3];
+};
+struct SpeciesConst {
+  double q_over_m, charge, dt;
+  int32_t massive, em, has_phi, do_deposit;
+};
+
+// counters: [0] alive after push, [1] absorbed inside, [2] absorbed outside, [3] overstep (most recent call);
+// [4] particle updates since grpic_create (cumulative)
+__device__ __forceinline__ void warp_count(unsigned long long* counters, int which, bool pred) {
+  const unsigned m = __ballot_sync(0xffffffffu, pred);
+  if (m && (threadIdx.x & 31) == 0) atomicAdd(&counters[which], (unsigned long long)__popc(m));
+}
+
+// global-memory field accessor
+template <typename T>
+struct GlobalFieldAcc {
+  const FPtrs<T>& F;
+  int64_t base;
+  int ld;
+  __device__ __forceinline__ T operator()(int c, int di, int dj) const {
+    return __ldg(F.f[c] + base + (int64_t)di * ld + dj);
+  }
+};
+
+// red.global.add: fire-and-forget reductions into the J arrays
+__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
+
+template <typename T>
+struct GlobalJSink {
+  const JPtrs<T>& J;
+  int64_t o[2];  // offsets of cells (ia,ja), (ib,jb)
+  int ld;
+  __device__ __forceinline__ void operator()(int s, T a0, T a1, T b0, T b1, T c00, T c10, T c01, T c11) const {
+    const int64_t k = o[s];
+    red_add(J.j[0] + k, a0);
+    red_add(J.j[0] + k + 1, a1);
+    red_add(J.j[1] + k, b0);
+    red_add(J.j[1] + k + ld, b1);
+    red_add(J.j[2] + k, c00);
+    red_add(J.j[2] + k + ld, c10);
+    red_add(J.j[2] + k + 1, c01);
+    red_add(J.j[2] + k + ld + 1, c11);
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
+// shared per-particle driver used by k_push / k_step_direct
+// ------------------------------------------------------------------------------------------------
+template <typename T, bool kDeposit>
+__device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
+                                                const JPtrs<T>& J, const SpeciesConst& sc,
+                                                unsigned long long* counters, int64_t k) {
+  const bool in_range = k < P.n;
+  const bool alive = in_range && P.tag[k] != 0;
+  int res = -1;
+  bool over = false;
+  if (alive) {
+    PState<T> p;
+    p.i1 = P.i1[k]; p.i2 = P.i2[k];
+    p.dx1 = P.dx1[k]; p.dx2 = P.dx2[k];
+    p.u1 = P.u1[k]; p.u2 = P.u2[k]; p.u3 = P.u3[k];
+    const int ia = p.i1, ja = p.i2;
+    const T xa = p.dx1, ya = p.dx2;
+    // step 1
+    P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya;
+    T Dp[3] = {T(0), T(0), T(0)}, Bp[3] = {T(0), T(0), T(0)};
+    const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
+    if (sc.em) {
+      GlobalFieldAcc<T> acc{F, cell, g.ld};
+      interp_fields(acc, p.dx1, p.dx2, Dp, Bp);          // step 2
+    }
+    const T eps = sc.massive ? T(1) : T(0);
+    const T dt = (T)sc.dt;
+    T dphidt;
+    bool reflected;
+    res = push_particle(g, p, sc.em != 0, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
+    P.i1[k] = p.i1; P.i2[k] = p.i2; P.dx1[k] = p.dx1; P.dx2[k] = p.dx2;
+    P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
+    if (sc.has_phi) P.phi[k] += dt * dphidt;
+    if (res != 0) P.tag[k] = 0;
+    if (kDeposit && sc.do_deposit && res == 0) {
+      const int di = p.i1 - ia, dj = p.i2 - ja;
+      if (di > 1 || di < -1 || dj > 1 || dj < -1) {
+        over = true;
+      } else {
+        T v3 = dphidt;
+        if (reflected)
+          v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
+                                   p.u2, p.u3, eps);
+        const T qw = (T)sc.charge * P.w[k];
+        GlobalJSink<T> sink{J, {cell, cell + (int64_t)di * g.ld + dj}, g.ld};
+        deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw / dt, qw, v3, sink);
+      }
+    }
+  }
+  warp_count(counters, 0, res == 0);
+  warp_count(counters, 1, res == 1);
+  warp_count(counters, 2, res == 2);
+  warp_count(counters, 4, res >= 0);
+  if (kDeposit) warp_count(counters, 3, over);
+}
+
+template <typename T, bool kDeposit>
+__global__ void __launch_bounds__(kBlock) k_push_or_step(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
+                                                         const JPtrs<T> J, const SpeciesConst sc,
+                                                         unsigned long long* counters) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  particle_direct<T, kDeposit>(g, P, F, J, sc, counters, k);
+}
+
+// deposit from stored (prev, current) — Eq. 36 velocity recomputed at the path midpoint as the paper
+// states it
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J,
+                                                    const SpeciesConst sc, unsigned long long* counters) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool over = false;
+  if (k < P.n && P.tag[k] != 0) {
+    const int ia = P.i1p[k], ja = P.i2p[k];
+    const int di = P.i1[k] - ia, dj = P.i2[k] - ja;
+    if (di > 1 || di < -1 || dj > 1 || dj < -1) {
+      over = true;
+    } else {
+      const T xa = P.dx1p[k], ya = P.dx2p[k], dx1 = P.dx1[k], dx2 = P.dx2[k];
+      const T eps = sc.massive ? T(1) : T(0);
+      const T v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + dx1), T(0.5) * (ya + (T)dj + dx2), P.u1[k],
+                                       P.u2[k], P.u3[k], eps);
+      const T qw = (T)sc.charge * P.w[k];
+      const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
+      GlobalJSink<T> sink{J, {cell, cell + (int64_t)di * g.ld + dj}, g.ld};
+      deposit_segments(di, dj, xa, ya, dx1, dx2, qw / (T)sc.dt, qw, v3, sink);
+    }
+  }
+  warp_count(counters, 3, over);
+}
+
+// ------------------------------------------------------------------------------------------------
+// counting sort by tile-major cell key
+// ------------------------------------------------------------------------------------------------
+struct SortGeom {
+  int32_t n1, n2, nt1, nt2;
+  uint32_t n_keys;  // nt1*nt2*kTile*kTile + 1 (the last key is "dead")
+};
+
+__device__ __forceinline__ uint32_t tile_key(const SortGeom& s, int i1, int i2, bool alive) {
+  if (!alive || i1 < 0 || i1 >= s.n1 || i2 < 0 || i2 >= s.n2) return s.n_keys - 1;
+  const uint32_t t1 = (uint32_t)i1 / kTile, l1 = (uint32_t)i1 % kTile;
+  const uint32_t t2 = (uint32_t)i2 / kTile, l2 = (uint32_t)i2 % kTile;
+  return ((t1 * s.nt2 + t2) * kTile + l1) * kTile + l2;
+}
+
+// histogram: one atomic per run of equal keys inside a warp (sorted input -> few runs)
+__global__ void __launch_bounds__(kBlock) k_sort_hist(const SortGeom s, int64_t n, const int32_t* i1,
+                                                      const int32_t* i2, const uint8_t* tag, uint32_t* key_out,
+                                                      uint32_t* hist) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool in = k < n;
+  uint32_t key = 0xffffffffu;
+  if (in) {
+    key = tile_key(s, i1[k], i2[k], tag[k] != 0);
+    key_out[k] = key;
+  }
+  const unsigned peers = __match_any_sync(0xffffffffu, key);
+  const int lane = threadIdx.x & 31;
+  if (in && lane == __ffs(peers) - 1) atomicAdd(&hist[key], (uint32_t)__popc(peers));
+}
+
+// destination slot of every particle: offset[key]++ (warp-aggregated)
+__global__ void __launch_bounds__(kBlock) k_sort_rank(int64_t n, const uint32_t* key_in, uint32_t* cursor,
+                                                      uint32_t* dest) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool in = k < n;
+  const uint32_t key = in ? key_in[k] : 0xffffffffu;
+  const unsigned peers = __match_any_sync(0xffffffffu, key);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  uint32_t base = 0;
+  if (in && lane == leader) base = atomicAdd(&cursor[key], (uint32_t)__popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (in) dest[k] = base + __popc(peers & ((1u << lane) - 1u));
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_sort_scatter(const PPtrs<T> in, const PPtrs<T> out,
+                                                         const uint32_t* dest) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= in.n) return;
+  const uint32_t d = dest[k];
+  out.i1[d] = in.i1[k]; out.i2[d] = in.i2[k];
+  out.dx1[d] = in.dx1[k]; out.dx2[d] = in.dx2[k];
+  out.u1[d] = in.u1[k]; out.u2[d] = in.u2[k]; out.u3[d] = in.u3[k];
+  if (in.phi) out.phi[d] = in.phi[k];
+  out.i1p[d] = in.i1p[k]; out.i2p[d] = in.i2p[k];
+  out.dx1p[d] = in.dx1p[k]; out.dx2p[d] = in.dx2p[k];
+  const_cast<T*>(out.w)[d] = in.w[k];
+  out.tag[d] = in.tag[k];
+}
+
+// exclusive scan of uint32 in three passes: 1024 threads x 4 items per block
+constexpr int kScanBlock = 1024;
+constexpr int kScanItems = 4;
+constexpr int kScanTile = kScanBlock * kScanItems;
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
+  __shared__ uint32_t warp_sums[32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  if (lane == 31) warp_sums[wid] = x;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t s = warp_sums[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+      if (lane >= o) s += y;
+    }
+    warp_sums[lane] = s;
+  }
+  __syncthreads();
+  const uint32_t warp_off = wid ? warp_sums[wid - 1] : 0u;
+  if (total) *total = warp_sums[31];
+  __syncthreads();
+  return warp_off + x - v;
+}
+
+__global__ void __launch_bounds__(kScanBlock) k_scan_local(uint32_t* data, uint32_t n, uint32_t* block_sums) {
+  const uint32_t base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+  uint32_t v[kScanItems], sum = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    v[j] = (base + j < n) ? data[base + j] : 0u;
+    sum += v[j];
+  }
+  uint32_t total;
+  uint32_t off = block_exclusive_scan(sum, &total);
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    if (base + j < n) data[base + j] = off;
+    off += v[j];
+  }
+  if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanBlock) k_scan_sums(uint32_t* block_sums, uint32_t nb) {
+  uint32_t carry = 0;
+  for (uint32_t start = 0; start < nb; start += kScanBlock) {
+    const uint32_t i = start + threadIdx.x;
+    const uint32_t v = (i < nb) ? block_sums[i] : 0u;
+    uint32_t total;
+    const uint32_t off = block_exclusive_scan(v, &total);
+    if (i < nb) block_sums[i] = carry + off;
+    carry += total;
+  }
+}
+
+__global__ void __launch_bounds__(kScanBlock) k_scan_add(uint32_t* data, uint32_t n, const uint32_t* block_sums) {
+  const uint32_t base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+  const uint32_t add = block_sums[blockIdx.x];
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j)
+    if (base + j < n) data[base + j] += add;
+}
+
+// Work items of the tiled step: (tile, first particle, count <= kChunk).  offsets[] is the scanned
+// histogram (n_keys + 1 entries, the last two delimit the dead particles).
+struct WorkItem {
+  uint32_t tile, begin, count, pad;
+};
+
+__global__ void k_items_count(const uint32_t* offsets, uint32_t n_tiles, uint32_t* n_items_of_tile) {
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_tiles) return;
+  const uint32_t cnt = offsets[(t + 1) * kTile * kTile] - offsets[t * kTile * kTile];
+  n_items_of_tile[t] = (cnt + kChunk - 1) / kChunk;
+}
+
+__global__ void k_items_fill(const uint32_t* offsets, uint32_t n_tiles, const uint32_t* item_offset_of_tile,
+                             WorkItem* items, uint32_t* n_items_out, uint32_t* n_alive_out) {
+  const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_tiles) return;
+  const uint32_t b = offsets[t * kTile * kTile], e = offsets[(t + 1) * kTile * kTile];
+  uint32_t k = item_offset_of_tile[t];
+  for (uint32_t s = b; s < e; s += kChunk) items[k++] = WorkItem{t, s, min((uint32_t)kChunk, e - s), 0u};
+  if (t == n_tiles - 1) {
+    *n_items_out = k;
+    *n_alive_out = e;
+  }
+}
+
+}  // namespace grpic

@@ -1,0 +1,277 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu).  Same seeded inputs on both sides; the
+oracle (FP64, CPU) is the reference; tolerances are north_star's (helpers.TOL).
+
+Every case runs the library through paper_2511_17701_b200.grpic (ctypes -> libgrpic_*.so)."""
+import numpy as np
+import pytest
+
+from helpers import TOL, compare_current, compare_particles, grid_from_domain, oracle_from_cols
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2511_17701_b200 import grpic
+    grpic.load("f32"); grpic.load("f64")       # fail loudly if the extension is missing
+    return grpic
+
+
+def _ctx(G, dom, prec, n_iter=10):
+    return G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec, n_iter=n_iter)
+
+
+def _zeros_J(G, ctx, prec):
+    import torch
+    return {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
+
+
+def _J_np(J):
+    return {k: v.detach().cpu().numpy().astype(np.float64) for k, v in J.items()}
+
+
+def _fields_both(G, wl, prec):
+    """device tensors for the GPU and the same (precision-rounded) values as FP64 numpy for the oracle"""
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    dev = G.grid_tensors(wl.fields, names, prec)
+    host = {k: dev[k].cpu().numpy().astype(np.float64) for k in names}
+    return dev, host
+
+
+def _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode, sort_first=False):
+    """One step of species `ps` on the GPU (mode: 'split' = interp_push + deposit, 'fused' = step),
+    the same step in the oracle from the GPU's own input state; returns the maxima."""
+    if sort_first:
+        ctx.sort(ps)
+    before = ps.to_numpy()
+    op = oracle_from_cols(O, before, ps.q_over_m, ps.charge, ps.massive)
+    J = _zeros_J(G, ctx, prec)
+    if mode == "split":
+        ctx.interp_push(ps, fdev, dt)
+        c_push = ctx.counters()
+        ctx.deposit(ps, J)
+        c = ctx.counters()
+        c.update({k: c_push[k] for k in ("alive", "absorbed_in", "absorbed_out")})
+    else:
+        ctx.step(ps, fdev, J, dt)
+        c = ctx.counters()
+    alive, a_in, a_out = O.push(g, op, fhost if ps.q_over_m != 0 and ps.massive else None, dt)
+    Jo, over = O.deposit(g, op, dt)
+    after = ps.to_numpy()
+    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2)
+    if res["n_idx_mismatch"] == 0:
+        assert (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"]) == (alive, a_in, a_out, over), (c, alive, a_in, a_out, over)
+        res.update(compare_current(Jo, _J_np(J), prec))
+    return res, c
+
+
+@pytest.mark.parametrize("mode", ["split", "fused"])
+def test_config1_tiny_f64_10_steps(G, O, W, mode):
+    """BASELINE config 1 at full size: Kerr a=0.9, 128x64, Wald field, 16 pairs-particles/cell, FP64, 10 steps.
+    Per-step parity (the oracle restarts every step from the GPU state), both species."""
+    wl = W.config_tiny()
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, "f64")
+    fdev, fhost = _fields_both(G, wl, "f64")
+    sets = [G.ParticleSet.from_host(sp, "f64") for sp in wl.species]
+    absorbed = 0
+    worst = dict(x_err=0.0, u_err=0.0, J3=0.0)
+    for step in range(wl.steps):
+        for ps in sets:
+            res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, "f64", mode)
+            absorbed += c["absorbed_in"] + c["absorbed_out"]
+            for k in worst:
+                worst[k] = max(worst[k], res[k])
+    assert absorbed > 0, "config 1 must exercise absorption inside the horizon"
+    print("config1", mode, worst, "absorbed", absorbed)
+
+
+def test_config1_tiled_path_f64(G, O, W):
+    """Same workload through grpic_sort + the shared-memory tile kernel, several steps between sorts."""
+    wl = W.config_tiny()
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, "f64")
+    fdev, fhost = _fields_both(G, wl, "f64")
+    sets = [G.ParticleSet.from_host(sp, "f64") for sp in wl.species]
+    for step in range(6):
+        for ps in sets:
+            _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, "f64", "fused", sort_first=(step % 3 == 0))
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_config2_geodesic_sample(G, O, W, prec):
+    """Config 2 (zero-field geodesics, a=0.95, q=0): a 2^17-particle sample against the oracle, 5 steps;
+    u_3 must come back bit-identical (Eq. 27: u~_3 = u_3)."""
+    wl = W.config_geodesic(n=1 << 17, dtype=prec)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    ps = G.ParticleSet.from_host(wl.species[0], prec)
+    u3_0 = ps.cols["u3"].clone()
+    for step in range(5):
+        res, c = _one_step_parity(G, O, ctx, g, ps, None, None, wl.dt, prec, "fused")
+    import torch
+    assert torch.equal(ps.cols["u3"], u3_0)
+    print("config2", prec, res)
+
+
+def _shrunk(W, name, shrink):
+    return dict(magnetosphere=W.config_magnetosphere, large=W.config_large, two_species=W.config_two_species)[name](shrink=shrink)
+
+
+@pytest.mark.parametrize("name,shrink,prec", [("magnetosphere", 8, "f32"), ("large", 16, "f32"),
+                                              ("two_species", 8, "f64"), ("two_species", 8, "f32")])
+@pytest.mark.parametrize("mode", ["split", "fused", "tiled"])
+def test_configs_3_4_5_shrunk(G, O, W, name, shrink, prec, mode):
+    """Configs 3-5 with both grid edges divided by `shrink` (per-cell counts, fields, dt recipe kept):
+    several tiles and a ragged tail; 3 steps per species."""
+    wl = _shrunk(W, name, shrink)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    fdev, fhost = _fields_both(G, wl, prec)
+    sets = [G.ParticleSet.from_host(sp, prec) for sp in wl.species]
+    worst = {}
+    for step in range(3):
+        for ps in sets:
+            res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, prec,
+                                      "fused" if mode == "tiled" else mode, sort_first=(mode == "tiled" and step == 0))
+            for k, v in res.items():
+                worst[k] = max(worst.get(k, 0), v)
+    print(name, prec, mode, worst)
+
+
+def test_sort_is_a_permutation_into_key_order(G, O, W):
+    import torch
+    wl = W.config_large(shrink=16)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, "f32")
+    sp = wl.species[0]
+    rng = np.random.default_rng(7)
+    perm = rng.permutation(sp.n)
+    for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "weight", "tag", "phi"):
+        setattr(sp, k, getattr(sp, k)[perm])
+    sp.tag = sp.tag.copy(); sp.tag[rng.random(sp.n) < 0.1] = 0
+    sp.weight = rng.random(sp.n) + 0.5
+    ps = G.ParticleSet.from_host(sp, "f32")
+    ps.cols["i1_prev"].copy_(torch.arange(sp.n, dtype=torch.int32))          # unique id to track the permutation
+    before = ps.to_numpy()
+    ctx.sort(ps)
+    after = ps.to_numpy()
+    ids = after["i1_prev"]
+    assert np.array_equal(np.sort(ids), np.arange(sp.n))                      # a permutation
+    for k, v in after.items():
+        if v is not None:
+            assert np.array_equal(v, before[k][ids]), k                       # every column moved alike
+    T = ctx.tile_size()
+    key, dead_key = O.sort_key(g, after["i1"], after["i2"], after["tag"], T)
+    assert np.all(np.diff(key) >= 0)                                          # non-decreasing key
+    assert np.all(after["tag"][: int((before["tag"] != 0).sum())] == 1)       # dead at the tail
+    ref, _, key_ref = O.sort_reference(g, oracle_from_cols(O, before, -1.0, -1.0, 1), T)
+    assert np.array_equal(key, key_ref)
+
+
+def test_step_host_matches_device_step(G, O, W):
+    import torch
+    wl = W.config_magnetosphere(shrink=8)
+    ctx = _ctx(G, wl.dom, "f32")
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    fdev = G.grid_tensors(wl.fields, names, "f32")
+    fhost = G.grid_tensors(wl.fields, names, "f32", device="cpu", pinned=True)
+    sp = wl.species[0]
+    pd = G.ParticleSet.from_host(sp, "f32")
+    ph = G.ParticleSet.from_host(sp, "f32", device="cpu", pinned=True)
+    Jd = _zeros_J(G, ctx, "f32")
+    Jh = {k: torch.zeros(ctx.shape, dtype=torch.float32).pin_memory() for k in ("J1", "J2", "J3")}
+    ctx.step(pd, fdev, Jd, wl.dt)
+    cd = ctx.counters()
+    up, down = ctx.step_host(ph, fhost, Jh, wl.dt)
+    ch = ctx.counters()
+    assert cd == ch
+    a, b = pd.to_numpy(), ph.to_numpy()
+    for k in a:
+        if a[k] is not None:
+            assert np.array_equal(a[k], b[k]), k
+    for k in Jd:
+        assert torch.allclose(Jd[k].cpu(), Jh[k], rtol=0, atol=1e-5 * float(Jd[k].abs().max()))
+    assert up > 0 and down > 0
+
+
+def test_edge_cases(G, O, W):
+    """n = 0; all dead; a particle crossing each axis (reflection); absorption at both radial edges; overstep."""
+    import torch
+    dom = W.Domain(32, 16, 0.9, 0.9 * W.horizon_radius(0.9), 20.0)
+    g = grid_from_domain(O, dom)
+    ctx = _ctx(G, dom, "f64")
+    fields = W.wald_fields(dom)
+    fdev = G.grid_tensors(fields, ("D1", "D2", "D3", "B1", "B2", "B3"), "f64")
+    fhost = {k: np.asarray(v, np.float64) for k, v in fields.items()}
+
+    class S:
+        pass
+
+    def mk(i1, i2, dx1, dx2, u1, u2, u3, tag=None, q=1.0):
+        s = S()
+        n = len(i1)
+        s.i1, s.i2 = np.array(i1, np.int32), np.array(i2, np.int32)
+        s.dx1, s.dx2 = np.array(dx1, float), np.array(dx2, float)
+        s.u1, s.u2, s.u3 = np.array(u1, float), np.array(u2, float), np.array(u3, float)
+        s.weight = np.ones(n); s.tag = np.ones(n, np.uint8) if tag is None else np.array(tag, np.uint8)
+        s.phi = np.zeros(n); s.q_over_m = q; s.charge = q; s.massive = 1
+        return s
+
+    # empty
+    ps = G.ParticleSet.from_host(mk([], [], [], [], [], [], []), "f64")
+    J = _zeros_J(G, ctx, "f64")
+    ctx.step(ps, fdev, J, 0.1); ctx.interp_push(ps, fdev, 0.1); ctx.deposit(ps, J); ctx.sort(ps)
+    assert ctx.counters() == dict(alive=0, absorbed_in=0, absorbed_out=0, overstep=0)
+    assert all(float(v.abs().max()) == 0 for v in J.values())
+    # all dead: nothing changes
+    s = mk([3, 4], [5, 6], [.1, .2], [.3, .4], [1, 2], [3, 4], [5, 6], tag=[0, 0])
+    ps = G.ParticleSet.from_host(s, "f64")
+    b = ps.to_numpy()
+    ctx.step(ps, fdev, J, 0.1)
+    a = ps.to_numpy()
+    assert all(np.array_equal(a[k], b[k]) for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "phi", "tag"))
+    assert all(float(v.abs().max()) == 0 for v in J.values())
+    # axis crossings, radial exits, an overstep (large u_2 near the horizon -> more than one cell in theta)
+    s = mk(i1=[10, 10, 0, 31, 12, 6], i2=[0, 15, 8, 8, 7, 8], dx1=[.5, .5, .01, .99, .5, .5],
+           dx2=[.02, .98, .5, .5, .5, .5],
+           u1=[0, 0, -3.0, 40.0, 0.1, 0.0], u2=[-1.5, 1.5, 0, 0, 0.2, 60.0], u3=[.05, .05, 1, 1, 0.3, 0.2])
+    for mode in ("split", "fused"):
+        ps = G.ParticleSet.from_host(s, "f64")
+        res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, 0.2, "f64", mode)
+        a = ps.to_numpy()
+        assert a["i2"][0] == 0 and a["u2"][0] > 0, "reflected at theta = 0"
+        assert a["i2"][1] == 15 and a["u2"][1] < 0, "reflected at theta = pi"
+        assert a["tag"][2] == 0 and a["i1"][2] < 0 and c["absorbed_in"] == 1
+        assert a["tag"][3] == 0 and a["i1"][3] >= 32 and c["absorbed_out"] == 1
+        assert c["overstep"] == 1 and c["alive"] == 4
+
+
+def test_abi_errors(G):
+    import ctypes as C
+    ctx = G.Context(16, 16, 0.5, 1.5, 10.0, precision="f32")
+    with pytest.raises(G.GrpicError):
+        ctx.set_int("n_iter", 0)
+    with pytest.raises(G.GrpicError):
+        ctx.set_int("nope", 1)
+    with pytest.raises(G.GrpicError):
+        ctx.set_real("small_angle", -1.0)
+    # deposit before any push -> ESTATE; charged species without fields -> EINVAL
+    import torch
+    z = lambda dt: torch.zeros(4, dtype=dt, device="cuda")
+    cols = {k: z(torch.int32) for k in ("i1", "i2", "i1_prev", "i2_prev")}
+    cols.update({k: z(torch.float32) for k in ("dx1", "dx2", "u1", "u2", "u3", "phi", "dx1_prev", "dx2_prev", "weight")})
+    cols["tag"] = torch.ones(4, dtype=torch.uint8, device="cuda")
+    ps = G.ParticleSet(cols, 1.0, 1.0, 1)
+    J = {k: torch.zeros(ctx.shape, device="cuda") for k in ("J1", "J2", "J3")}
+    with pytest.raises(G.GrpicError) as e:
+        ctx.deposit(ps, J)
+    assert e.value.code == G.GRPIC_ESTATE
+    with pytest.raises(G.GrpicError) as e:
+        ctx.interp_push(ps, None, 0.1)
+    assert e.value.code == G.GRPIC_EINVAL
+    with pytest.raises(G.GrpicError) as e:
+        ctx.step(ps, None, J, -1.0)
+    assert e.value.code == G.GRPIC_EINVAL
