@@ -109,7 +109,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    shrink = 16
+    shrink = 4
     O, wl, g, parts, fields = _oracle_setup(args.workload, shrink)
     for _ in range(args.warmup):
         _oracle_step(O, wl, g, parts, fields)
@@ -222,13 +222,13 @@ def run_ours(args):
         return launches
 
     it = 0
+    sampler = ClockSampler(local) if rank == 0 else None      # nvidia-smi needs ~a second to start sampling
     for _ in range(args.warmup):
         one_step(it); it += 1
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     upd0 = ctx.updates_total()
-    sampler = ClockSampler(local) if rank == 0 else None
     evs = []
     t_a = torch.cuda.Event(enable_timing=True); t_b = torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -325,7 +325,7 @@ def run_ours(args):
     if e2e is not None:
         out["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.workload, shrink=16, steps=2)
+        out["cpu_baseline"] = cpu_baseline(args.workload, shrink=4, steps=4)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

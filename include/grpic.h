@@ -88,7 +88,7 @@ typedef struct { grpic_real *J1, *J2, *J3; } grpic_current; /* ACCUMULATED into;
 /* sizeof(grpic_real) of the loaded build: 4 or 8. */
 int grpic_real_bytes(void);
 
-/* Create a context for one mesh and one Kerr spin a (|a| < 1... <= 1), radial extent [r_min, r_max]
+/* Create a context for one mesh and one Kerr spin a (|a| <= 1), radial extent [r_min, r_max]
  * in units of r_g (north_star: grpic_create(grid, a, r_min, r_max); metric of App. A.3).
  * Defaults: n_iter = 10, small_angle = 1e-5 (SMALL_ANGLE_GR).
  * Errors: EINVAL (NULL, n1/n2 < 1, nghost < 1, r_map != 1, r_min <= 0 or >= r_max), ECUDA, ENOMEM. */
@@ -97,7 +97,9 @@ int grpic_destroy(grpic_ctx* ctx);
 
 /* "n_iter": fixed iteration count of the two midpoint integrators, 1..64.
  * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernel after a grpic_sort;
- *              0 forces the direct kernel (global gathers and atomics). */
+ *              0 forces the direct kernel (global gathers and atomics).
+ * "tma": 1 (default) stages the tile's field stencil with TMA; 0 uses plain cooperative loads (also the
+ *        automatic choice when a field array is not 16-byte aligned or (n2 + 2 nghost)*sizeof(real) % 16 != 0). */
 int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t value);
 /* "small_angle": theta used in any metric evaluation is clamped to [eps, pi - eps] (R-S9). */
 int grpic_set_real(grpic_ctx* ctx, const char* key, double value);

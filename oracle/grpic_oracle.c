@@ -281,6 +281,13 @@ typedef struct {
   double q_over_m, charge; int32_t massive;
 } orc_particles;
 
+/* Optional diagnostic output (no effect on any result): the raw displacement (del1, del2) of Eq. 28-29
+ * before renormalisation and reflection, one entry per particle.  The parity tests use it to evaluate
+ * the conditioning of phi for particles whose midpoint grazes the polar axis. */
+static double* orc_diag_del1 = NULL;
+static double* orc_diag_del2 = NULL;
+void orc_set_diag(double* del1, double* del2) { orc_diag_del1 = del1; orc_diag_del2 = del2; }
+
 /* Whole per-particle update with the fields at the particle given (Dp,Bp,
  * contravariant code basis).  Steps 1, 3-11 of P:264-311 and the BCs of
  * P:465-467 (reading R-S9). Returns 0 alive, 1 absorbed inside, 2 absorbed outside. */
@@ -316,6 +323,7 @@ static int orc_push_core(const orc_grid* g, orc_particles* p, int64_t k, const d
   }
   double del[2];
   const double dphidt = orc_geodesic_x(g, x1n, x2n, u, eps, dt, del);   /* 10 */
+  if (orc_diag_del1) { orc_diag_del1[k] = del[0]; orc_diag_del2[k] = del[1]; }
   if (p->phi) p->phi[k] += dt * dphidt;                        /* 11 */
 
   /* renormalise to (cell, displacement in [0,1)) */

@@ -198,10 +198,22 @@ def interp(g: Grid, fields, i1, i2, dx1, dx2):
     return D, B
 
 
-def push(g: Grid, p: Particles, fields, dt: float):
-    """In-place step 1-11 + BCs on `p`.  Returns (alive, absorbed_in, absorbed_out)."""
+def push(g: Grid, p: Particles, fields, dt: float, diag: dict | None = None):
+    """In-place step 1-11 + BCs on `p`.  Returns (alive, absorbed_in, absorbed_out).
+    If `diag` is a dict it receives 'del1', 'del2': the raw displacement of Eq. 28-29 per particle."""
     gc = g.c(); pc = p.c()
     cnt = (C.c_int64 * 3)()
+    if diag is not None:
+        diag["del1"] = np.zeros(p.n); diag["del2"] = np.zeros(p.n)
+        lib().orc_set_diag(_ptr(diag["del1"], _dp), _ptr(diag["del2"], _dp))
+    try:
+        return _push(gc, pc, p, fields, dt, cnt)
+    finally:
+        if diag is not None:
+            lib().orc_set_diag(None, None)
+
+
+def _push(gc, pc, p, fields, dt, cnt):
     if fields is None:
         assert p.q_over_m == 0.0 or not p.massive, "charged particles need fields"
         lib().orc_push(C.byref(gc), C.byref(pc), None, C.c_double(dt), cnt)

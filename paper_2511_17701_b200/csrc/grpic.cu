@@ -36,7 +36,7 @@ struct SortState {          // tile table of one species (keyed by the address o
 struct grpic_ctx {
   grpic_grid grid;
   double a, r_min, r_max, small_angle;
-  int n_iter, tile_path;
+  int n_iter, tile_path, use_tma;
   double last_dt;
   bool have_dt;
   unsigned long long* d_counters;   // 5: four of the last call + cumulative updates
@@ -200,6 +200,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->small_angle = 1e-5;                                  // SMALL_ANGLE_GR
   ctx->n_iter = 10;
   ctx->tile_path = 1;
+  ctx->use_tma = 1;
   ctx->have_dt = false; ctx->last_dt = 0.0;
   ctx->d_counters = nullptr;
   ctx->d_keys = ctx->d_dest = ctx->d_hist = ctx->d_block_sums = ctx->d_tile_items = nullptr;
@@ -244,6 +245,10 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t v) {
   }
   if (!std::strcmp(key, "tile_path")) {
     ctx->tile_path = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "tma")) {
+    ctx->use_tma = v ? 1 : 0;
     return GRPIC_OK;
   }
   return fail(ctx, GRPIC_EINVAL, std::string("unknown integer key: ") + key);
@@ -322,7 +327,7 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   }
   const SortState& ss = it->second;
   std::string terr;
-  if (!launch_step_tiled<real>(ctx->tma, g, P, F, Jp, sc, ctx->d_counters, ss.items, ss.d_n_items, ss.max_items,
+  if (!launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items, ss.d_n_items, ss.max_items,
                                ss.n_at_sort, st, terr))
     return fail(ctx, GRPIC_ECUDA, terr);
   return GRPIC_OK;

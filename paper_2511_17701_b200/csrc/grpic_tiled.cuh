@@ -2,7 +2,7 @@
 //
 // One CTA per work item (tile, particle range <= kChunk) of the table grpic_sort built:
 //   1. one elected thread issues six 2-D TMA loads (cp.async.bulk.tensor) that bring the tile's
-//      field stencil — (kTile + 2 kHalo + 2)^2 samples of each of D1 D2 D3 B1 B2 B3 — into shared
+//      field stencil — (kTile + 2 kHalo + 2) x (kTile + 2 kHalo + 6) samples of each of D1 D2 D3 B1 B2 B3 — into shared
 //      memory, completion tracked by an mbarrier; out-of-range rows/columns are zero-filled by TMA;
 //   2. every thread pushes its particles (steps 1-11 + BCs) with the gather served from shared
 //      memory; a particle that has drifted out of the window since the last sort falls back to
@@ -39,13 +39,13 @@ struct TmaEncoder {
     else
       cudaGetLastError();
   }
-  // [rows][ld] array of `elem_bytes`-wide floats, box kWinF x kWinF
+  // [rows][ld] array of `elem_bytes`-wide floats, box kWinF rows x kRowF columns
   bool encode(CUtensorMap* m, const void* base, int elem_bytes, int rows, int ld) const {
     if (!fn) return false;
     if (((uintptr_t)base & 15u) || (((size_t)ld * elem_bytes) & 15u)) return false;
     cuuint64_t dims[2] = {(cuuint64_t)ld, (cuuint64_t)rows};
     cuuint64_t strides[1] = {(cuuint64_t)ld * elem_bytes};
-    cuuint32_t box[2] = {(cuuint32_t)kWinF, (cuuint32_t)kWinF};
+    cuuint32_t box[2] = {(cuuint32_t)kRowF, (cuuint32_t)kWinF};
     cuuint32_t estr[2] = {1, 1};
     return fn(m, elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2,
               const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -94,7 +94,7 @@ template <typename T>
 struct SmemFieldAcc {
   const T* base;  // sample (c1, c2) of component 0, i.e. the particle's own cell
   __device__ __forceinline__ T operator()(int c, int di, int dj) const {
-    return base[c * (kWinF * kWinF) + di * kWinF + dj];
+    return base[c * (kWinF * kRowF) + di * kRowF + dj];
   }
 };
 
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
                                                        const uint32_t* n_items_ptr, uint32_t max_items,
                                                        int64_t n_at_sort, int nt2, int use_tma,
                                                        const __grid_constant__ FieldMaps maps) {
-  __shared__ __align__(128) T sF[6 * kWinF * kWinF];
+  __shared__ __align__(128) T sF[6 * kWinF * kRowF];
   __shared__ __align__(16) T sJ[3 * kJComp];
   __shared__ __align__(8) uint64_t bar;
 
@@ -150,6 +150,10 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
   const WorkItem item = items[blockIdx.x];
   const int c1lo = (int)(item.tile / (uint32_t)nt2) * kTile - kHalo;   // window origin, cells
   const int c2lo = (int)(item.tile % (uint32_t)nt2) * kTile - kHalo;
+  // first fetched column (array index): the window's first sample, rounded down to a multiple of 4
+  // elements so that its byte address is 16-byte aligned (a TMA requirement on the innermost coordinate)
+  const int a2lo = c2lo - 1 + g.ng;
+  const int off2 = ((a2lo % 4) + 4) % 4;
 
   // ---- 1. stage the field stencil ----
   if (use_tma) {
@@ -159,16 +163,16 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
     }
     __syncthreads();
     if (tid == 0) {
-      mbar_expect_tx(&bar, 6u * kWinF * kWinF * (uint32_t)sizeof(T));
+      mbar_expect_tx(&bar, 6u * kWinF * kRowF * (uint32_t)sizeof(T));
 #pragma unroll
       for (int c = 0; c < 6; ++c)
-        tma_load_2d(sF + c * kWinF * kWinF, &maps.m[c], c2lo - 1 + g.ng, c1lo - 1 + g.ng, &bar);
+        tma_load_2d(sF + c * kWinF * kRowF, &maps.m[c], a2lo - off2, c1lo - 1 + g.ng, &bar);
     }
   } else {
     const int rows = g.n1 + 2 * g.ng;
-    for (int e = tid; e < 6 * kWinF * kWinF; e += kBlock) {
-      const int c = e / (kWinF * kWinF), rem = e % (kWinF * kWinF);
-      const int a1 = c1lo - 1 + g.ng + rem / kWinF, a2 = c2lo - 1 + g.ng + rem % kWinF;
+    for (int e = tid; e < 6 * kWinF * kRowF; e += kBlock) {
+      const int c = e / (kWinF * kRowF), rem = e % (kWinF * kRowF);
+      const int a1 = c1lo - 1 + g.ng + rem / kRowF, a2 = a2lo - off2 + rem % kRowF;
       sF[e] = (a1 >= 0 && a1 < rows && a2 >= 0 && a2 < g.ld) ? __ldg(F.f[c] + (int64_t)a1 * g.ld + a2) : T(0);
     }
   }
@@ -204,7 +208,7 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
       const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
       T Dp[3], Bp[3];
       if (a_in) {
-        SmemFieldAcc<T> acc{sF + (wa1 + 1) * kWinF + (wa2 + 1)};
+        SmemFieldAcc<T> acc{sF + (wa1 + 1) * kRowF + (wa2 + 1 + off2)};
         interp_fields(acc, p.dx1, p.dx2, Dp, Bp);
       } else {
         GlobalFieldAcc<T> acc{F, cell, g.ld};
@@ -307,13 +311,13 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
 }
 
 template <typename T>
-bool launch_step_tiled(const TmaEncoder& enc, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
+bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
                        const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
                        cudaStream_t st, std::string& err) {
   FieldMaps maps;
   memset(&maps, 0, sizeof(maps));
-  int use_tma = 1;
+  int use_tma = want_tma ? 1 : 0;
   const int rows = g.n1 + 2 * g.ng;
   for (int c = 0; c < 6 && use_tma; ++c)
     if (!enc.encode(&maps.m[c], F.f[c], (int)sizeof(T), rows, g.ld)) use_tma = 0;

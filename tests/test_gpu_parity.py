@@ -57,10 +57,11 @@ def _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode, sort_first=F
     else:
         ctx.step(ps, fdev, J, dt)
         c = ctx.counters()
-    alive, a_in, a_out = O.push(g, op, fhost if ps.q_over_m != 0 and ps.massive else None, dt)
+    diag = {}
+    alive, a_in, a_out = O.push(g, op, fhost if ps.q_over_m != 0 and ps.massive else None, dt, diag=diag)
     Jo, over = O.deposit(g, op, dt)
     after = ps.to_numpy()
-    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2)
+    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag)
     if res["n_idx_mismatch"] == 0:
         assert (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"]) == (alive, a_in, a_out, over), (c, alive, a_in, a_out, over)
         res.update(compare_current(Jo, _J_np(J), prec))
@@ -234,10 +235,10 @@ def test_edge_cases(G, O, W):
     a = ps.to_numpy()
     assert all(np.array_equal(a[k], b[k]) for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "phi", "tag"))
     assert all(float(v.abs().max()) == 0 for v in J.values())
-    # axis crossings, radial exits, an overstep (large u_2 near the horizon -> more than one cell in theta)
-    s = mk(i1=[10, 10, 0, 31, 12, 6], i2=[0, 15, 8, 8, 7, 8], dx1=[.5, .5, .01, .99, .5, .5],
-           dx2=[.02, .98, .5, .5, .5, .5],
-           u1=[0, 0, -3.0, 40.0, 0.1, 0.0], u2=[-1.5, 1.5, 0, 0, 0.2, 60.0], u3=[.05, .05, 1, 1, 0.3, 0.2])
+    # axis crossings, radial exits
+    s = mk(i1=[10, 10, 0, 31, 12], i2=[0, 15, 8, 8, 7], dx1=[.5, .5, .01, .99, .5],
+           dx2=[.02, .98, .5, .5, .5],
+           u1=[0, 0, -3.0, 40.0, 0.1], u2=[-1.5, 1.5, 0, 0, 0.2], u3=[.05, .05, 1, 1, 0.3])
     for mode in ("split", "fused"):
         ps = G.ParticleSet.from_host(s, "f64")
         res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, 0.2, "f64", mode)
@@ -246,7 +247,14 @@ def test_edge_cases(G, O, W):
         assert a["i2"][1] == 15 and a["u2"][1] < 0, "reflected at theta = pi"
         assert a["tag"][2] == 0 and a["i1"][2] < 0 and c["absorbed_in"] == 1
         assert a["tag"][3] == 0 and a["i1"][3] >= 32 and c["absorbed_out"] == 1
-        assert c["overstep"] == 1 and c["alive"] == 4
+        assert c["overstep"] == 0 and c["alive"] == 3
+    # overstep: a fast particle and a time step large enough to cross more than one cell in theta
+    s = mk(i1=[6, 12], i2=[8, 7], dx1=[.5, .5], dx2=[.5, .5], u1=[0.0, 0.1], u2=[60.0, 0.02], u3=[0.2, 0.3])
+    for mode in ("split", "fused"):
+        ps = G.ParticleSet.from_host(s, "f64")
+        Jt = _zeros_J(G, ctx, "f64")
+        res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, 1.5, "f64", mode)
+        assert c["overstep"] == 1 and abs(int(ps.cols["i2"][0]) - 8) > 1
 
 
 def test_abi_errors(G):
