@@ -96,6 +96,9 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
 int grpic_destroy(grpic_ctx* ctx);
 
 /* "n_iter": fixed iteration count of the two midpoint integrators, 1..64.
+ * "early_exit": 1 (default) leaves a fixed-point loop as soon as an iterate repeats the previous one bit
+ *              for bit — every later iterate would be that same value, so the result IS the one of
+ *              n_iter iterations; 0 always executes all n_iter (used by the test that proves this).
  * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernel after a grpic_sort;
  *              0 forces the direct kernel (global gathers and atomics).
  * "tma": 1 (default) stages the tile's field stencil with TMA; 0 uses plain cooperative loads (also the

@@ -36,7 +36,7 @@ struct SortState {          // tile table of one species (keyed by the address o
 struct grpic_ctx {
   grpic_grid grid;
   double a, r_min, r_max, small_angle;
-  int n_iter, tile_path, use_tma;
+  int n_iter, tile_path, use_tma, early_exit;
   double last_dt;
   bool have_dt;
   unsigned long long* d_counters;   // 5: four of the last call + cumulative updates
@@ -84,10 +84,14 @@ Consts<real> make_consts(const grpic_ctx* c) {
   g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
   g.log_rmin = (real)std::log(c->r_min);
   g.dxi = (real)dxi; g.deta = (real)deta;
-  g.half_dxi = (real)(0.5 * dxi); g.half_deta = (real)(0.5 * deta);
+  g.inv_dxi = (real)(1.0 / dxi);
   g.inv_deta2 = (real)(1.0 / (deta * deta));
   g.th_min = (real)c->small_angle;
   g.th_max = (real)(M_PI - c->small_angle);
+  g.sin_min = (real)std::sin((double)g.th_min);
+  g.cos_min = (real)std::cos((double)g.th_min);
+  g.early_exit = c->early_exit;
+  g.pad2_ = 0;
   return g;
 }
 
@@ -201,6 +205,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->n_iter = 10;
   ctx->tile_path = 1;
   ctx->use_tma = 1;
+  ctx->early_exit = 1;
   ctx->have_dt = false; ctx->last_dt = 0.0;
   ctx->d_counters = nullptr;
   ctx->d_keys = ctx->d_dest = ctx->d_hist = ctx->d_block_sums = ctx->d_tile_items = nullptr;
@@ -245,6 +250,10 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t v) {
   }
   if (!std::strcmp(key, "tile_path")) {
     ctx->tile_path = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "early_exit")) {
+    ctx->early_exit = v ? 1 : 0;
     return GRPIC_OK;
   }
   if (!std::strcmp(key, "tma")) {

@@ -24,9 +24,12 @@ struct Consts {
   T a, a2;           // spin and its square
   T log_rmin;        // xi at x1 = 0
   T dxi, deta;       // d(xi)/d(x1), d(theta)/d(x2)
-  T half_dxi, half_deta;
+  T inv_dxi;         // 1/dxi
   T inv_deta2;       // 1/deta^2
   T th_min, th_max;  // [small_angle, pi - small_angle]
+  T sin_min, cos_min;  // sin, cos of th_min
+  int32_t early_exit;  // leave a fixed-point loop once the iterate repeats bit for bit (identical result)
+  int32_t pad2_;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -94,7 +97,7 @@ struct Coord<double> {
 
 template <>
 struct Coord<float> {
-  float r0, thp, sgn;  // r at x, theta' at x (unclamped), +1 (upper half) or -1 (mirrored)
+  float r0, thp, s0, c0, sgn;  // r, theta', sin(theta'), cos(theta') at x (theta' unclamped); +1 or -1 (mirrored)
   __device__ __forceinline__ void init(const Consts<float>& g, int i1, float dx1, int i2, float dx2) {
     const float xi = fmaf(dx1, g.dxi, fmaf((float)i1, g.dxi, g.log_rmin));
     r0 = expf(xi);
@@ -105,21 +108,34 @@ struct Coord<float> {
       thp = ((float)i2 + dx2) * g.deta;
       sgn = 1.f;
     }
+    sincosf(thp, &s0, &c0);
   }
   __device__ __forceinline__ void at(const Consts<float>& g, float h1, float h2, float& r, float& sth,
                                      float& cth) const {
-    // exp(e) for |e| <= dxi/2 + (a cell or two): 5th-order Taylor, |e|^6/720 < 1e-9 for |e| < 0.1
+    // r0 * exp(e), |e| = |h1| dxi: 4th-order Taylor (|e|^5/120 < 1e-9 for |e| < 0.04), expf beyond
     const float e = h1 * g.dxi;
-    float p = fmaf(e, 1.f / 120.f, 1.f / 24.f);
-    p = fmaf(p, e, 1.f / 6.f);
+    float p = fmaf(e, 1.f / 24.f, 1.f / 6.f);
     p = fmaf(p, e, 0.5f);
     p = fmaf(p, e, 1.f);
     p = fmaf(p, e, 1.f);
-    r = (fabsf(e) < 0.1f) ? r0 * p : r0 * expf(e);
-    float th = fmaf(sgn * h2, g.deta, thp);
-    th = fminf(fmaxf(th, g.th_min), g.th_max);
+    r = (fabsf(e) < 0.04f) ? r0 * p : r0 * expf(e);
+    // sin, cos(theta' + d) by angle addition, |d| = |h2| deta: sin d to d^3, cos d to d^4
+    // (relative errors d^4/120, d^6/720 < 4e-8 for |d| < 0.045); sincosf beyond
+    const float d = sgn * h2 * g.deta;
+    const float th = thp + d;
     float s, c;
-    sincosf(th, &s, &c);
+    if (fabsf(d) < 0.045f) {
+      const float d2 = d * d;
+      const float sd = fmaf(d * d2, -1.f / 6.f, d);
+      const float cd = fmaf(d2, fmaf(d2, 1.f / 24.f, -0.5f), 1.f);
+      s = fmaf(s0, cd, c0 * sd);
+      c = fmaf(c0, cd, -s0 * sd);
+    } else {
+      sincosf(th, &s, &c);
+    }
+    // axis regularisation: theta' clamped to [th_min, th_max]
+    if (th < g.th_min) { s = g.sin_min; c = g.cos_min; }
+    if (th > g.th_max) { s = g.sin_min; c = -g.cos_min; }
     sth = s;
     cth = sgn * c;
   }
@@ -130,7 +146,8 @@ struct Coord<float> {
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 struct MetricLite {
-  T alpha, beta1, hu11, hu22, hu33, hu13;
+  T ia2;   // 1/alpha^2 = 1 + z
+  T beta1, hu11, hu22, hu33, hu13;
 };
 
 template <typename T>
@@ -138,19 +155,27 @@ __device__ __forceinline__ void metric_lite(const Consts<T>& g, T r, T sth, T ct
   const T r2 = r * r;
   const T s2th = sth * sth;
   const T Sigma = fma_(g.a2 * cth, cth, r2);
-  const T Delta = r2 - T(2) * r + g.a2;
+  const T Delta = fma_(r, r - T(2), g.a2);
   const T r2a2 = r2 + g.a2;
-  const T A = r2a2 * r2a2 - g.a2 * Delta * s2th;
-  const T Sp2r = Sigma + T(2) * r;              // Sigma (1 + z)
+  const T A = fma_(-(g.a2 * s2th), Delta, r2a2 * r2a2);
+  const T Sp2r = fma_(T(2), r, Sigma);          // Sigma (1 + z)
   const T iS = rcp_(Sigma);
   const T iSp2r = rcp_(Sp2r);
-  const T is1 = rcp_(g.dxi * r);                // 1/s1
-  m.alpha = sqrt_(Sigma * iSp2r);               // (1+z)^-1/2
-  m.beta1 = T(2) * r * iSp2r * is1;             // z/(1+z)/s1
-  m.hu11 = A * iS * iSp2r * is1 * is1;
+  const T is1 = g.inv_dxi * rcp_(r);            // 1/s1
+  const T q = iS * is1;
+  m.ia2 = Sp2r * iS;
+  m.beta1 = (T(2) * r) * (iSp2r * is1);         // z/(1+z)/s1
+  m.hu11 = (A * iSp2r) * (q * is1);
   m.hu22 = iS * g.inv_deta2;
   m.hu33 = iS * rcp_(s2th);
-  m.hu13 = g.a * iS * is1;
+  m.hu13 = g.a * q;
+}
+
+// 1/u^0 = alpha/gamma at a midpoint (Eq. 20 with footnote 8)
+template <typename T>
+__device__ __forceinline__ T inv_u0(const MetricLite<T>& m, T u1sq, T u2sq, T u3sq, T u1u3x2, T eps) {
+  const T g2 = fma_(m.hu11, u1sq, fma_(m.hu22, u2sq, fma_(m.hu33, u3sq, fma_(m.hu13, u1u3x2, eps))));
+  return rsqrt_(g2 * m.ia2);
 }
 
 // Full set at x^(n): adds h_ij (for the tetrad) and the twelve derivatives of Eq. 27.
@@ -209,12 +234,6 @@ __device__ __forceinline__ void metric_full(const Consts<T>& g, T r, T sth, T ct
   const T al3 = m.alpha * m.alpha * m.alpha;
   m.d_alpha[0] = -w * iS2 * al3;
   m.d_alpha[1] = r * d2S * iS2 * al3;
-}
-
-// Eq. 20: gamma^2 = eps + h^{ij} u_i u_j
-template <typename T, typename M>
-__device__ __forceinline__ T gamma2(const M& m, T u1, T u2, T u3, T eps) {
-  return eps + m.hu11 * u1 * u1 + m.hu22 * u2 * u2 + m.hu33 * u3 * u3 + T(2) * m.hu13 * u1 * u3;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -373,8 +392,13 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
         const T hiu0 = T(0.5) * m.alpha * igam;           // 1/(2 u^0)
         const T q0 = f0c + ub0 * (m.d_hu11[0] * ub0 + d13u3_0) + m.d_hu22[0] * ub1 * ub1;
         const T q1 = f1c + ub0 * (m.d_hu11[1] * ub0 + d13u3_1) + m.d_hu22[1] * ub1 * ub1;
-        ut0 = us0 + dt * (-gam * m.d_alpha[0] + ub0 * m.d_beta1[0] - hiu0 * q0);
-        ut1 = us1 + dt * (-gam * m.d_alpha[1] + ub0 * m.d_beta1[1] - hiu0 * q1);
+        const T nt0 = us0 + dt * (-gam * m.d_alpha[0] + ub0 * m.d_beta1[0] - hiu0 * q0);
+        const T nt1 = us1 + dt * (-gam * m.d_alpha[1] + ub0 * m.d_beta1[1] - hiu0 * q1);
+        // the map is deterministic: once an iterate repeats bit for bit every later one equals it
+        const bool fixed = (nt0 == ut0) && (nt1 == ut1);
+        ut0 = nt0;
+        ut1 = nt1;
+        if (fixed && g.early_exit) break;
       }
       u[0] = ut0;
       u[1] = ut1;
@@ -388,22 +412,31 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
   // step 10, Eq. 28-29 in displacement space: del = x~ - x^(n); all coefficients at x^(n) + del/2
   T del1 = T(0), del2 = T(0);
   MetricLite<T> mm;
+  T iu0 = T(0);
+  const T u1sq = u[0] * u[0], u2sq = u[1] * u[1], u3sq = u[2] * u[2], u1u3x2 = T(2) * u[0] * u[2];
+  bool fixed = false;
   for (int it = 0; it < g.n_iter; ++it) {
     T r, sth, cth;
     X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
     metric_lite(g, r, sth, cth, mm);
-    const T iu0 = mm.alpha * rsqrt_(gamma2(mm, u[0], u[1], u[2], eps));   // 1/u^0
-    del1 = dt * ((mm.hu11 * u[0] + mm.hu13 * u[2]) * iu0 - mm.beta1);
-    del2 = dt * (mm.hu22 * u[1] * iu0);
+    iu0 = inv_u0(mm, u1sq, u2sq, u3sq, u1u3x2, eps);
+    const T n1 = dt * ((mm.hu11 * u[0] + mm.hu13 * u[2]) * iu0 - mm.beta1);
+    const T n2 = dt * (mm.hu22 * u[1] * iu0);
+    // bit-identical iterate => every later iterate is the same: stopping here IS n_iter iterations
+    fixed = (n1 == del1) && (n2 == del2);
+    del1 = n1;
+    del2 = n2;
+    if (fixed && g.early_exit) break;
   }
-  // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2
-  {
+  // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2.  If the last iterate repeated, the midpoint
+  // of the last evaluation is x_m itself and its coefficients are reused; otherwise evaluate there.
+  if (!fixed) {
     T r, sth, cth;
     X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
     metric_lite(g, r, sth, cth, mm);
-    const T iu0 = mm.alpha * rsqrt_(gamma2(mm, u[0], u[1], u[2], eps));
-    dphidt = (mm.hu13 * u[0] + mm.hu33 * u[2]) * iu0;
+    iu0 = inv_u0(mm, u1sq, u2sq, u3sq, u1u3x2, eps);
   }
+  dphidt = (mm.hu13 * u[0] + mm.hu33 * u[2]) * iu0;
   // renormalise to (cell, displacement in [0,1))
   T t1 = p.dx1 + del1, t2 = p.dx2 + del2;
   const T f1 = floor_(t1), f2 = floor_(t2);
@@ -471,7 +504,7 @@ __device__ __forceinline__ T v3_at_path_midpoint(const Consts<T>& g, int ia, int
   X.at(g, T(0), T(0), r, sth, cth);
   MetricLite<T> mm;
   metric_lite(g, r, sth, cth, mm);
-  const T iu0 = mm.alpha * rsqrt_(gamma2(mm, u1, u2, u3, eps));
+  const T iu0 = inv_u0(mm, u1 * u1, u2 * u2, u3 * u3, T(2) * u1 * u3, eps);
   return (mm.hu13 * u1 + mm.hu33 * u3) * iu0;
 }
 

@@ -128,8 +128,32 @@ __device__ __forceinline__ void global_add8(const JPtrs<T>& J, int64_t k, int ld
   red_add(J.j[2] + k + ld + 1, v[7]);
 }
 
+// Warp-aggregated flush of the per-lane run accumulators into the shared J tile: lanes holding the same
+// cell key in consecutive lanes form a run; the run is summed with log2(32) shuffle steps and its first
+// lane issues the eight shared atomics.  (Shared FP atomics are compare-and-swap loops on sm_100a —
+// ATOMS.CAST.SPIN — so fewer, conflict-free atomics is what matters.)
 template <typename T>
-__global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
+__device__ __forceinline__ void warp_flush_runs(T* sJ, int lane, bool valid, int node, T acc[8]) {
+  const int key = valid ? node : (0x40000000 + lane);                 // idle lanes: unique keys
+  const int key_prev = __shfl_up_sync(0xffffffffu, key, 1);
+  const bool head = (lane == 0) || (key != key_prev);
+  const unsigned heads = __ballot_sync(0xffffffffu, head);
+  const unsigned above = heads & ~((2u << lane) - 1u);                // run heads strictly above my lane
+  const int run_last = above ? (__ffs(above) - 2) : 31;               // last lane of my run
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const bool take = (lane + d) <= run_last;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const T o = __shfl_down_sync(0xffffffffu, acc[q], d);
+      if (take) acc[q] += o;
+    }
+  }
+  if (head && valid) smem_add8(sJ, node, acc);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
                                                        const JPtrs<T> J, const SpeciesConst sc,
                                                        unsigned long long* counters, const WorkItem* items,
                                                        const uint32_t* n_items_ptr, uint32_t max_items,
@@ -186,9 +210,20 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
   const T inv_dt = T(1) / dt;
   const uint32_t end = item.begin + item.count;
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
-  for (uint32_t base = item.begin + (tid & ~31); base < end; base += kBlock) {
+  // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): different warps then work on
+  // different cells, and consecutive iterations of one lane stay in the same cell, so contributions
+  // are first accumulated per lane in registers (acc) and flushed only when some lane changes cell.
+  const uint32_t per_warp = ((item.count + kBlock - 1) / kBlock) * 32u;
+  const uint32_t w_begin = item.begin + (uint32_t)(tid >> 5) * per_warp;
+  const uint32_t w_end = min(end, w_begin + per_warp);
+  bool acc_valid = false;
+  int acc_node = 0;
+  T acc[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) acc[q] = T(0);
+  for (uint32_t base = w_begin; base < w_end; base += 32u) {
     const uint32_t k = base + lane;
-    const bool alive = k < end && P.tag[k] != 0;
+    const bool alive = k < w_end && P.tag[k] != 0;
     int res = -1;
     bool dep_smem = false, dep_cross = false;
     int node_a = 0x7fffffff, node_b = 0;
@@ -259,29 +294,23 @@ __global__ void __launch_bounds__(kBlock) k_step_tiled(const Consts<T> g, const 
       }
       n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
     }
-    // ---- warp-aggregated shared atomics: runs of equal node_a are summed with shuffles ----
-    const unsigned any_smem = __ballot_sync(0xffffffffu, dep_smem);
-    if (any_smem) {
-      const int key = dep_smem ? node_a : (0x40000000 + lane);          // non-depositing lanes: unique keys
-      const int key_prev = __shfl_up_sync(0xffffffffu, key, 1);
-      const bool head = (lane == 0) || (key != key_prev);
-      const unsigned heads = __ballot_sync(0xffffffffu, head);
-      // last lane of my run
-      const unsigned above = heads & ~((2u << lane) - 1u);              // heads strictly above my lane
-      const int run_last = above ? (__ffs(above) - 2) : 31;
+    // ---- run accumulation: flush (warp-aggregated) when any lane leaves its cell ----
+    const bool must_flush = acc_valid && (!dep_smem || node_a != acc_node);
+    if (__any_sync(0xffffffffu, must_flush)) {
+      warp_flush_runs(sJ, lane, acc_valid, acc_node, acc);
+      acc_valid = false;
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const bool take = (lane + d) <= run_last;
+      for (int q = 0; q < 8; ++q) acc[q] = T(0);
+    }
+    if (dep_smem) {
+      acc_valid = true;
+      acc_node = node_a;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          const T o = __shfl_down_sync(0xffffffffu, va[q], d);
-          if (take) va[q] += o;
-        }
-      }
-      if (head && dep_smem) smem_add8(sJ, node_a, va);
+      for (int q = 0; q < 8; ++q) acc[q] += va[q];
       if (dep_cross) smem_add8(sJ, node_b, vb);
     }
   }
+  if (__any_sync(0xffffffffu, acc_valid)) warp_flush_runs(sJ, lane, acc_valid, acc_node, acc);
   // counters: one atomic per warp and counter
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {

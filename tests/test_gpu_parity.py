@@ -283,3 +283,28 @@ def test_abi_errors(G):
     with pytest.raises(G.GrpicError) as e:
         ctx.step(ps, None, J, -1.0)
     assert e.value.code == G.GRPIC_EINVAL
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_early_exit_is_bit_identical_to_all_iterations(G, W, prec):
+    """A fixed-point loop that stops when an iterate repeats bit for bit returns exactly what n_iter
+    iterations return (the map is deterministic).  Proven by running both on the same inputs."""
+    import torch
+    wl = W.config_large(shrink=16)
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    fdev = G.grid_tensors(wl.fields, names, prec)
+    outs = []
+    for ee in (1, 0):
+        ctx = _ctx(G, wl.dom, prec)
+        ctx.set_int("early_exit", ee)
+        ps = G.ParticleSet.from_host(wl.species[1], prec)
+        J = _zeros_J(G, ctx, prec)
+        for _ in range(3):
+            ctx.step(ps, fdev, J, wl.dt)
+        outs.append((ps.to_numpy(), _J_np(J)))
+    a, b = outs
+    for k in a[0]:
+        if a[0][k] is not None:
+            assert np.array_equal(a[0][k], b[0][k]), k
+    for k in a[1]:
+        assert np.allclose(a[1][k], b[1][k], rtol=0, atol=TOL[prec]["J"] * np.abs(b[1][k]).max())
