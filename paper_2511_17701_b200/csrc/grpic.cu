@@ -78,7 +78,6 @@ Consts<real> make_consts(const grpic_ctx* c) {
   Consts<real> g;
   g.n1 = c->grid.n1; g.n2 = c->grid.n2; g.ng = c->grid.nghost; g.n_iter = c->n_iter;
   g.ld = c->grid.n2 + 2 * c->grid.nghost;
-  g.pad_ = 0;
   const double dxi = std::log(c->r_max / c->r_min) / c->grid.n1;
   const double deta = M_PI / c->grid.n2;
   g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
@@ -90,8 +89,9 @@ Consts<real> make_consts(const grpic_ctx* c) {
   g.th_max = (real)(M_PI - c->small_angle);
   g.sin_min = (real)std::sin((double)g.th_min);
   g.cos_min = (real)std::cos((double)g.th_min);
+  g.sin_max = (real)std::sin((double)g.th_max);
+  g.cos_max = (real)std::cos((double)g.th_max);
   g.early_exit = c->early_exit;
-  g.pad2_ = 0;
   return g;
 }
 

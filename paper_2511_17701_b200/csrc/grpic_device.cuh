@@ -7,6 +7,13 @@
 // All metric quantities are recomputed in registers from (cell, displacement, spin, map constants);
 // nothing is tabulated.  Notation follows App. A: Sigma, Delta, A, z, alpha, beta^1,
 // h^{ij} ("hu"), h_{ij} ("hd"), code basis of the log-r map A.3 with s1 = dxi*r, s2 = deta.
+//
+// The formulas are the paper's, rearranged so that the two fixed-point loops (Eq. 26-29) execute as few
+// instructions as possible:
+//   - with s1 = dxi*r the shift is beta^1 = (2/dxi)/(Sigma+2r), and alpha/gamma = Sigma * rsqrt((Sigma+2r) G)
+//     with G = Sigma*gamma^2, so 1/Sigma is never formed inside the coordinate loop;
+//   - everything that does not change between iterations (u-dependent products, dt factors, the
+//     derivative terms that multiply u_3) is folded before the loops.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -19,29 +26,27 @@ namespace grpic {
 template <typename T>
 struct Consts {
   int32_t n1, n2, ng, n_iter;
-  int32_t ld;        // row length of every grid array: n2 + 2*ng
-  int32_t pad_;
-  T a, a2;           // spin and its square
-  T log_rmin;        // xi at x1 = 0
-  T dxi, deta;       // d(xi)/d(x1), d(theta)/d(x2)
-  T inv_dxi;         // 1/dxi
-  T inv_deta2;       // 1/deta^2
-  T th_min, th_max;  // [small_angle, pi - small_angle]
-  T sin_min, cos_min;  // sin, cos of th_min
+  int32_t ld;          // row length of every grid array: n2 + 2*ng
   int32_t early_exit;  // leave a fixed-point loop once the iterate repeats bit for bit (identical result)
-  int32_t pad2_;
+  T a, a2;             // spin and its square
+  T log_rmin;          // xi at x1 = 0
+  T dxi, deta;         // d(xi)/d(x1), d(theta)/d(x2)
+  T inv_dxi;           // 1/dxi
+  T inv_deta2;         // 1/deta^2
+  T th_min, th_max;    // [small_angle, pi - small_angle]
+  T sin_min, cos_min;  // sin, cos of th_min
+  T sin_max, cos_max;  // sin, cos of th_max (FP64: the values the plain formula gives at the clamped angle)
 };
 
 // ------------------------------------------------------------------------------------------------
 // scalar helpers: IEEE operators in FP64; hardware approximations (<= 2 ulp) in FP32
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double rcp_(double x) { return 1.0 / x; }
-__device__ __forceinline__ double rsqrt_(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
 __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
-__device__ __forceinline__ double exp_(double x) { return exp(x); }
-__device__ __forceinline__ void sincos_(double x, double* s, double* c) { sincos(x, s, c); }
 __device__ __forceinline__ double floor_(double x) { return floor(x); }
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ double abs_(double x) { return fabs(x); }
 __device__ __forceinline__ double below_one(double) { return 0x1.fffffffffffffp-1; }
 
 __device__ __forceinline__ float rcp_(float x) {
@@ -59,39 +64,102 @@ __device__ __forceinline__ float sqrt_(float x) {
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ float exp_(float x) { return expf(x); }
-__device__ __forceinline__ void sincos_(float x, float* s, float* c) { sincosf(x, s, c); }
 __device__ __forceinline__ float floor_(float x) { return floorf(x); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ float below_one(float) { return 0x1.fffffep-1f; }
+
+// exp(e) - 1 ... as 1 + e + ... and sin(d), cos(d) for the small in-step displacements of the midpoint
+// iteration.  Truncation errors (relative): FP32 |e| < 0.04: e^5/120 < 1e-9; |d| < 0.045: d^4/120, d^6/720 < 4e-8.
+// FP64 |e| < 0.04: e^11/11! < 2e-23; |d| < 0.045: d^12/12!, d^13/13! < 2e-25.
+__device__ __forceinline__ float exp_small(float e) {
+  float p = fmaf(e, 1.f / 24.f, 1.f / 6.f);
+  p = fmaf(p, e, 0.5f);
+  p = fmaf(p, e, 1.f);
+  return fmaf(p, e, 1.f);
+}
+__device__ __forceinline__ void sincos_small(float d, float& sd, float& cd) {
+  const float d2 = d * d;
+  sd = fmaf(d * d2, -1.f / 6.f, d);
+  cd = fmaf(d2, fmaf(d2, 1.f / 24.f, -0.5f), 1.f);
+}
+__device__ __forceinline__ double exp_small(double e) {
+  double p = fma(e, 1.0 / 3628800.0, 1.0 / 362880.0);
+  p = fma(p, e, 1.0 / 40320.0);
+  p = fma(p, e, 1.0 / 5040.0);
+  p = fma(p, e, 1.0 / 720.0);
+  p = fma(p, e, 1.0 / 120.0);
+  p = fma(p, e, 1.0 / 24.0);
+  p = fma(p, e, 1.0 / 6.0);
+  p = fma(p, e, 0.5);
+  p = fma(p, e, 1.0);
+  return fma(p, e, 1.0);
+}
+__device__ __forceinline__ void sincos_small(double d, double& sd, double& cd) {
+  const double d2 = d * d;
+  double p = fma(d2, -1.0 / 39916800.0, 1.0 / 362880.0);
+  p = fma(p, d2, -1.0 / 5040.0);
+  p = fma(p, d2, 1.0 / 120.0);
+  p = fma(p, d2, -1.0 / 6.0);
+  sd = fma(p * d2, d, d);
+  double q = fma(d2, -1.0 / 3628800.0, 1.0 / 40320.0);
+  q = fma(q, d2, -1.0 / 720.0);
+  q = fma(q, d2, 1.0 / 24.0);
+  q = fma(q, d2, -0.5);
+  cd = fma(q, d2, 1.0);
+}
+template <typename T> struct SmallLimits;
+template <> struct SmallLimits<float> { static constexpr float e = 0.04f, d = 0.045f; };
+template <> struct SmallLimits<double> { static constexpr double e = 0.04, d = 0.045; };
 
 // ------------------------------------------------------------------------------------------------
 // Coordinate map (r0 = 0, h0 = 0) and the axis regularisation (R-S9).
 //
-// FP64: the plain formulas, x = i + dx, r = exp(ln r_min + x1*dxi), theta = x2*deta.
-// FP32: the same map evaluated so that rounding does not eat the in-cell displacement:
-//   - theta is measured from the NEARER axis (theta' = pi - theta on the lower half, exact in the
-//     integer part), so that sin(theta) keeps full relative accuracy next to theta = pi;
-//   - a midpoint x + h is reached from the stored r, theta' by r*exp(h1*dxi), theta' +- h2*deta,
-//     never by re-adding i + dx + h in FP32 (ulp(2048) = 2.4e-4 cells).
+// r, sin(theta), cos(theta) at x^(n) are evaluated once with the library functions; a midpoint
+// x^(n) + h is then reached by r0*exp(h1*dxi) and the angle-addition formulas with short polynomials
+// in the small displacement (library functions beyond SmallLimits).
+// FP64: theta = (x2 + h2)*deta is formed exactly as the plain formula forms it, so that the
+//   ill-conditioned sin(theta) next to theta = pi sees the same rounded angle.
+// FP32: theta is measured from the NEARER axis (theta' = pi - theta on the lower half, exact in the
+//   integer part) so that sin(theta) keeps full relative accuracy next to theta = pi, and a midpoint is
+//   never formed by re-adding i + dx + h in FP32 (ulp(2048) = 2.4e-4 cells).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 struct Coord;
 
 template <>
 struct Coord<double> {
-  double x1, x2;
-  __device__ __forceinline__ void init(const Consts<double>&, int i1, double dx1, int i2, double dx2) {
-    x1 = (double)i1 + dx1;
+  double x2, r0, th0, s0, c0;
+  __device__ __forceinline__ void init(const Consts<double>& g, int i1, double dx1, int i2, double dx2) {
+    const double x1 = (double)i1 + dx1;
     x2 = (double)i2 + dx2;
+    r0 = exp(g.log_rmin + x1 * g.dxi);
+    th0 = x2 * g.deta;
+    sincos(th0, &s0, &c0);
   }
-  // r, sin(theta), cos(theta) at x + (h1, h2)
+  // r, sin(theta), cos(theta) at x^(n) itself (theta clamped)
+  __device__ __forceinline__ void at0(const Consts<double>& g, double& r, double& sth, double& cth) const {
+    r = r0; sth = s0; cth = c0;
+    if (th0 < g.th_min) { sth = g.sin_min; cth = g.cos_min; }
+    if (th0 > g.th_max) { sth = g.sin_max; cth = g.cos_max; }
+  }
   __device__ __forceinline__ void at(const Consts<double>& g, double h1, double h2, double& r, double& sth,
                                      double& cth) const {
-    r = exp(g.log_rmin + (x1 + h1) * g.dxi);
-    double th = (x2 + h2) * g.deta;
-    th = fmin(fmax(th, g.th_min), g.th_max);
-    sincos(th, &sth, &cth);
+    const double e = h1 * g.dxi;
+    const double th = (x2 + h2) * g.deta;
+    const double d = th - th0;
+    if (fabs(e) < SmallLimits<double>::e && fabs(d) < SmallLimits<double>::d) {
+      r = r0 * exp_small(e);
+      double sd, cd;
+      sincos_small(d, sd, cd);
+      sth = fma(s0, cd, c0 * sd);
+      cth = fma(c0, cd, -s0 * sd);
+    } else {
+      r = r0 * exp(e);
+      sincos(th, &sth, &cth);
+    }
+    if (th < g.th_min) { sth = g.sin_min; cth = g.cos_min; }
+    if (th > g.th_max) { sth = g.sin_max; cth = g.cos_max; }
   }
 };
 
@@ -110,27 +178,26 @@ struct Coord<float> {
     }
     sincosf(thp, &s0, &c0);
   }
+  __device__ __forceinline__ void at0(const Consts<float>& g, float& r, float& sth, float& cth) const {
+    float s = s0, c = c0;
+    if (thp < g.th_min) { s = g.sin_min; c = g.cos_min; }
+    if (thp > g.th_max) { s = g.sin_min; c = -g.cos_min; }
+    r = r0; sth = s; cth = sgn * c;
+  }
   __device__ __forceinline__ void at(const Consts<float>& g, float h1, float h2, float& r, float& sth,
                                      float& cth) const {
-    // r0 * exp(e), |e| = |h1| dxi: 4th-order Taylor (|e|^5/120 < 1e-9 for |e| < 0.04), expf beyond
     const float e = h1 * g.dxi;
-    float p = fmaf(e, 1.f / 24.f, 1.f / 6.f);
-    p = fmaf(p, e, 0.5f);
-    p = fmaf(p, e, 1.f);
-    p = fmaf(p, e, 1.f);
-    r = (fabsf(e) < 0.04f) ? r0 * p : r0 * expf(e);
-    // sin, cos(theta' + d) by angle addition, |d| = |h2| deta: sin d to d^3, cos d to d^4
-    // (relative errors d^4/120, d^6/720 < 4e-8 for |d| < 0.045); sincosf beyond
-    const float d = sgn * h2 * g.deta;
+    const float d = (sgn * g.deta) * h2;
     const float th = thp + d;
     float s, c;
-    if (fabsf(d) < 0.045f) {
-      const float d2 = d * d;
-      const float sd = fmaf(d * d2, -1.f / 6.f, d);
-      const float cd = fmaf(d2, fmaf(d2, 1.f / 24.f, -0.5f), 1.f);
+    if (fabsf(e) < SmallLimits<float>::e && fabsf(d) < SmallLimits<float>::d) {
+      r = r0 * exp_small(e);
+      float sd, cd;
+      sincos_small(d, sd, cd);
       s = fmaf(s0, cd, c0 * sd);
       c = fmaf(c0, cd, -s0 * sd);
     } else {
+      r = r0 * expf(e);
       sincosf(th, &s, &c);
     }
     // axis regularisation: theta' clamped to [th_min, th_max]
@@ -142,102 +209,131 @@ struct Coord<float> {
 };
 
 // ------------------------------------------------------------------------------------------------
-// Metric.  "Lite": what Eq. 29/30 need at a midpoint.
+// Midpoint evaluation of Eq. 29/30: everything Eq. 29 needs from the metric at (r, sin theta),
+// for a fixed u.  With w1 = u_1/s1, U2 = u_2/s2 (physical-basis covariant components):
+//   G = Sigma gamma^2 = eps Sigma + A w1^2/(Sigma+2r) + U2^2 + u_3^2/sin^2 + 2 a w1 u_3      (Eq. 20)
+//   1/u^0 = alpha/gamma = Sigma R,   R = rsqrt((Sigma + 2r) G)
+//   dx^1/dt = (h^11 u_1 + h^13 u_3)/u^0 - beta^1 = [(A w1/(Sigma+2r) + a u_3)/r * R - 2/(Sigma+2r)]/dxi
+//   dx^2/dt = h^22 u_2/u^0 = (u_2/deta^2) R
+//   dphi/dt = (h^13 u_1 + h^33 u_3)/u^0 = (a w1 + u_3/sin^2) R
 // ------------------------------------------------------------------------------------------------
 template <typename T>
-struct MetricLite {
-  T ia2;   // 1/alpha^2 = 1 + z
-  T beta1, hu11, hu22, hu33, hu13;
+struct MidU {           // per-particle constants of the coordinate loop
+  T w1c;                // u_1/dxi          (w1 = w1c / r)
+  T U2sq;               // (u_2/deta)^2
+  T u3, u3sq, au3, c2au3;
+  T k1, k2;             // dt/dxi,  dt u_2/deta^2
+  T eps;
+  __device__ __forceinline__ void init(const Consts<T>& g, T u1, T u2, T u3_, T eps_, T dt) {
+    w1c = u1 * g.inv_dxi;
+    U2sq = (u2 * u2) * g.inv_deta2;
+    u3 = u3_;
+    u3sq = u3_ * u3_;
+    au3 = g.a * u3_;
+    c2au3 = au3 + au3;
+    k1 = dt * g.inv_dxi;
+    k2 = (dt * u2) * g.inv_deta2;
+    eps = eps_;
+  }
 };
 
 template <typename T>
-__device__ __forceinline__ void metric_lite(const Consts<T>& g, T r, T sth, T cth, MetricLite<T>& m) {
-  const T r2 = r * r;
-  const T s2th = sth * sth;
-  const T Sigma = fma_(g.a2 * cth, cth, r2);
-  const T Delta = fma_(r, r - T(2), g.a2);
-  const T r2a2 = r2 + g.a2;
-  const T A = fma_(-(g.a2 * s2th), Delta, r2a2 * r2a2);
-  const T Sp2r = fma_(T(2), r, Sigma);          // Sigma (1 + z)
-  const T iS = rcp_(Sigma);
-  const T iSp2r = rcp_(Sp2r);
-  const T is1 = g.inv_dxi * rcp_(r);            // 1/s1
-  const T q = iS * is1;
-  m.ia2 = Sp2r * iS;
-  m.beta1 = (T(2) * r) * (iSp2r * is1);         // z/(1+z)/s1
-  m.hu11 = (A * iSp2r) * (q * is1);
-  m.hu22 = iS * g.inv_deta2;
-  m.hu33 = iS * rcp_(s2th);
-  m.hu13 = g.a * q;
-}
+struct MidEval {
+  T R, w1, is2;
+  // returns the two displacement rates times dt
+  __device__ __forceinline__ void eval(const Consts<T>& g, const MidU<T>& U, T r, T sth, T& n1, T& n2) {
+    const T r2 = r * r;
+    const T a2s2 = g.a2 * (sth * sth);
+    const T r2a2 = r2 + g.a2;
+    const T Sigma = r2a2 - a2s2;
+    const T Sp2r = fma_(T(2), r, Sigma);
+    const T Delta = fma_(r, r - T(2), g.a2);
+    const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
+    const T ir = rcp_(r);
+    const T iSp2r = rcp_(Sp2r);
+    is2 = rcp_(sth * sth);
+    w1 = U.w1c * ir;
+    const T t = (A * iSp2r) * w1;
+    T G = fma_(U.eps, Sigma, U.U2sq);
+    G = fma_(t, w1, G);
+    G = fma_(U.u3sq, is2, G);
+    G = fma_(U.c2au3, w1, G);
+    R = rsqrt_(Sp2r * G);
+    n1 = U.k1 * fma_((t + U.au3) * ir, R, T(-2) * iSp2r);
+    n2 = U.k2 * R;
+  }
+  __device__ __forceinline__ T dphidt(const Consts<T>& g, const MidU<T>& U) const {
+    return fma_(g.a, w1, U.u3 * is2) * R;
+  }
+};
 
-// 1/u^0 = alpha/gamma at a midpoint (Eq. 20 with footnote 8)
-template <typename T>
-__device__ __forceinline__ T inv_u0(const MetricLite<T>& m, T u1sq, T u2sq, T u3sq, T u1u3x2, T eps) {
-  const T g2 = fma_(m.hu11, u1sq, fma_(m.hu22, u2sq, fma_(m.hu33, u3sq, fma_(m.hu13, u1u3x2, eps))));
-  return rsqrt_(g2 * m.ia2);
-}
-
-// Full set at x^(n): adds h_ij (for the tetrad) and the twelve derivatives of Eq. 27.
+// ------------------------------------------------------------------------------------------------
+// Full set at x^(n): tetrad coefficients and the Eq. 27 coefficients, with the analytic
+// derivatives of App. A (general rule P:772-778; A.2 list P:814-816; the A.3 extras from
+// s1 = dxi*exp(xi) depending on x1; corrections R-S2) written in logarithmic form:
+//   d h^22 = -h^22 dSigma/Sigma;  d h^33 = -h^33 (dSigma/Sigma + 2 cot(theta) dtheta);
+//   d h^13 = -h^13 (dSigma/Sigma + dxi [x1 only]);  d beta^1 = -beta^1 (dSigma + 2 s1 [x1 only])/(Sigma+2r);
+//   d alpha = (r dSigma - Sigma dr)/((Sigma+2r)^2 alpha);
+//   d h^11 = dA/(Sigma (Sigma+2r) s1^2) - h^11 (dSigma/Sigma + (dSigma + 2 s1 [x1])/(Sigma+2r) + 2 dxi [x1]).
+// ------------------------------------------------------------------------------------------------
 template <typename T>
 struct MetricFull {
-  T alpha, beta1, hu11, hu22, hu33, hu13;
+  T alpha, hu11, hu22, hu33, hu13;
   T hd22, hd33, hd13;
   T d_alpha[2], d_beta1[2], d_hu11[2], d_hu22[2], d_hu33[2], d_hu13[2];  // [0] = d/dx1, [1] = d/dx2
 };
 
-// Derivatives: chain rule on the closed forms above (general rule P:772-778; A.2 list P:814-816;
-// the A.3 extras from s1 = dxi*exp(xi) depending on x1; corrections R-S2).
 template <typename T>
 __device__ __forceinline__ void metric_full(const Consts<T>& g, T r, T sth, T cth, MetricFull<T>& m) {
   const T a = g.a, a2 = g.a2;
   const T r2 = r * r;
   const T s2th = sth * sth;
-  const T Sigma = fma_(a2 * cth, cth, r2);
-  const T Delta = r2 - T(2) * r + a2;
+  const T a2s2 = a2 * s2th;
   const T r2a2 = r2 + a2;
-  const T A = r2a2 * r2a2 - a2 * Delta * s2th;
-  const T Sp2r = Sigma + T(2) * r;
-  const T s1 = g.dxi * r, s2 = g.deta;
-  const T iS = rcp_(Sigma), iSp2r = rcp_(Sp2r), is1 = rcp_(s1), is2th = rcp_(s2th);
-  const T iS2 = iS * iS;
-  const T opz = Sp2r * iS;                       // 1 + z
-  m.alpha = sqrt_(Sigma * iSp2r);
-  m.beta1 = T(2) * r * iSp2r * is1;
-  m.hu11 = A * iS * iSp2r * is1 * is1;
+  const T Sigma = fma_(a2 * cth, cth, r2);
+  const T Delta = fma_(r, r - T(2), a2);
+  const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
+  const T Sp2r = fma_(T(2), r, Sigma);
+  const T s1 = g.dxi * r;
+  const T iS = rcp_(Sigma), iSp2r = rcp_(Sp2r), is2th = rcp_(s2th);
+  const T is1 = g.inv_dxi * rcp_(r);
+  const T al2 = Sigma * iSp2r;                   // alpha^2 = 1/(1+z)
+  const T ial = rsqrt_(al2);
+  m.alpha = al2 * ial;
+  const T beta1 = (T(2) * g.inv_dxi) * iSp2r;
+  const T B = (iS * iSp2r) * (is1 * is1);        // 1/(Sigma (Sigma+2r) s1^2)
+  m.hu11 = A * B;
   m.hu22 = iS * g.inv_deta2;
   m.hu33 = iS * is2th;
-  m.hu13 = a * iS * is1;
-  m.hd22 = s2 * s2 * Sigma;
-  m.hd33 = A * s2th * iS;
-  m.hd13 = -s1 * a * opz * s2th;
+  m.hu13 = (a * iS) * is1;
+  m.hd22 = (g.deta * g.deta) * Sigma;
+  m.hd33 = (A * s2th) * iS;
+  m.hd13 = -(s1 * a) * ((Sp2r * iS) * s2th);
 
-  const T d1S = T(2) * r * s1;
-  const T d2S = T(-2) * a2 * sth * cth * s2;
-  const T d1D = T(2) * (r - T(1)) * s1;
-  const T d1A = T(4) * r * s1 * r2a2 - a2 * s2th * d1D;
-  const T d2A = d2S * Delta;                     // -2 a^2 sin cos Delta s2
-  const T iP = iS * iSp2r;                       // 1/(Sigma (Sigma + 2r))
-  const T iP2s = iP * iP * is1 * is1;
-  const T P = Sigma * Sp2r;
-  m.d_hu11[0] = (P * d1A - T(2) * A * (r * d1S + Sigma * (d1S + s1))) * iP2s - T(2) * g.dxi * m.hu11;
-  m.d_hu11[1] = (P * d2A - T(2) * A * d2S * (r + Sigma)) * iP2s;
-  m.d_hu22[0] = -d1S * iS2 * g.inv_deta2;
-  m.d_hu22[1] = -d2S * iS2 * g.inv_deta2;
-  m.d_hu33[0] = -d1S * iS2 * is2th;
-  m.d_hu33[1] = T(-2) * cth * s2 * iS2 * is2th * rcp_(sth) * (Sigma - a2 * s2th);
-  m.d_hu13[0] = -a * is1 * d1S * iS2 - g.dxi * m.hu13;
-  m.d_hu13[1] = -a * is1 * d2S * iS2;
-  const T w = s1 * Sigma - r * d1S;              // Sigma^2/2 * d1 z
-  m.d_beta1[0] = T(2) * is1 * w * iSp2r * iSp2r - g.dxi * m.beta1;
-  m.d_beta1[1] = T(-2) * is1 * r * d2S * iSp2r * iSp2r;
-  const T al3 = m.alpha * m.alpha * m.alpha;
-  m.d_alpha[0] = -w * iS2 * al3;
-  m.d_alpha[1] = r * d2S * iS2 * al3;
+  const T d1S = (T(2) * r) * s1;
+  const T d2S = (T(-2) * a2 * g.deta) * (sth * cth);
+  const T d1A = (T(4) * r * s1) * r2a2 - a2s2 * ((T(2) * (r - T(1))) * s1);
+  const T d2A = d2S * Delta;
+  const T l1S = d1S * iS, l2S = d2S * iS;        // d ln Sigma
+  const T l1P = (d1S + T(2) * s1) * iSp2r;       // d ln (Sigma + 2r)
+  const T l2P = d2S * iSp2r;
+  m.d_hu11[0] = fma_(B, d1A, -m.hu11 * (l1S + l1P + T(2) * g.dxi));
+  m.d_hu11[1] = fma_(B, d2A, -m.hu11 * (l2S + l2P));
+  m.d_hu22[0] = -m.hu22 * l1S;
+  m.d_hu22[1] = -m.hu22 * l2S;
+  m.d_hu33[0] = -m.hu33 * l1S;
+  m.d_hu33[1] = -m.hu33 * fma_((T(2) * g.deta) * cth, rcp_(sth), l2S);
+  m.d_hu13[0] = -m.hu13 * (l1S + g.dxi);
+  m.d_hu13[1] = -m.hu13 * l2S;
+  m.d_beta1[0] = -beta1 * l1P;
+  m.d_beta1[1] = -beta1 * l2P;
+  const T ka = (iSp2r * iSp2r) * ial;            // 1/((Sigma+2r)^2 alpha)
+  m.d_alpha[0] = fma_(r, d1S, -Sigma * s1) * ka;
+  m.d_alpha[1] = (r * d2S) * ka;
 }
 
 // ------------------------------------------------------------------------------------------------
-// Tetrad at x^(n): matrix form of P:754 (R-S3).  e[] caches the square roots.
+// Tetrad at x^(n): matrix form of P:754 (R-S3).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 struct Tetrad {
@@ -254,91 +350,80 @@ struct Tetrad {
   __device__ __forceinline__ void cntrv_to_tetrad(const T A[3], T Ah[3]) const {
     Ah[0] = A[0] * isq11;
     Ah[1] = sq22 * A[1];
-    Ah[2] = k13 * A[0] + sq33 * A[2];
+    Ah[2] = fma_(k13, A[0], sq33 * A[2]);
   }
   __device__ __forceinline__ void cov_to_tetrad(const T u[3], T uh[3]) const {
-    uh[0] = sq11 * (u[0] - k13 * isq33 * u[2]);
+    uh[0] = sq11 * fma_(-(k13 * isq33), u[2], u[0]);
     uh[1] = u[1] * isq22;
     uh[2] = u[2] * isq33;
   }
   __device__ __forceinline__ void tetrad_to_cov(const T uh[3], T u[3]) const {
-    u[0] = uh[0] * isq11 + k13 * uh[2];
+    u[0] = fma_(uh[0], isq11, k13 * uh[2]);
     u[1] = sq22 * uh[1];
     u[2] = sq33 * uh[2];
   }
 };
 
 // Boris rotation over dt/2 in the orthonormal frame (coefficient c = (q/m) alpha dt/4, R-S5).
+// cD = c*D-hat, cB = c*B-hat.
 template <typename T>
-__device__ __forceinline__ void boris_half(const T Dh[3], const T Bh[3], T c, T uh[3]) {
-  const T um0 = uh[0] + c * Dh[0], um1 = uh[1] + c * Dh[1], um2 = uh[2] + c * Dh[2];
-  const T ig = c * rsqrt_(T(1) + um0 * um0 + um1 * um1 + um2 * um2);
-  const T t0 = Bh[0] * ig, t1 = Bh[1] * ig, t2 = Bh[2] * ig;
-  const T f = T(2) * rcp_(T(1) + t0 * t0 + t1 * t1 + t2 * t2);
+__device__ __forceinline__ void boris_half(const T cD[3], const T cB[3], T uh[3]) {
+  const T um0 = uh[0] + cD[0], um1 = uh[1] + cD[1], um2 = uh[2] + cD[2];
+  const T ig = rsqrt_(fma_(um0, um0, fma_(um1, um1, fma_(um2, um2, T(1)))));
+  const T t0 = cB[0] * ig, t1 = cB[1] * ig, t2 = cB[2] * ig;
+  const T f = T(2) * rcp_(fma_(t0, t0, fma_(t1, t1, fma_(t2, t2, T(1)))));
   const T s0 = f * t0, s1 = f * t1, s2 = f * t2;
-  const T p0 = um0 + (um1 * t2 - um2 * t1);
-  const T p1 = um1 + (um2 * t0 - um0 * t2);
-  const T p2 = um2 + (um0 * t1 - um1 * t0);
-  uh[0] = um0 + (p1 * s2 - p2 * s1) + c * Dh[0];
-  uh[1] = um1 + (p2 * s0 - p0 * s2) + c * Dh[1];
-  uh[2] = um2 + (p0 * s1 - p1 * s0) + c * Dh[2];
+  const T p0 = um0 + fma_(um1, t2, -um2 * t1);
+  const T p1 = um1 + fma_(um2, t0, -um0 * t2);
+  const T p2 = um2 + fma_(um0, t1, -um1 * t0);
+  uh[0] = (um0 + fma_(p1, s2, -p2 * s1)) + cD[0];
+  uh[1] = (um1 + fma_(p2, s0, -p0 * s2)) + cD[1];
+  uh[2] = (um2 + fma_(p0, s1, -p1 * s0)) + cD[2];
 }
 
 // ------------------------------------------------------------------------------------------------
 // Field gather (step 2; scheme R-S4): every Yee component is first averaged to the four
-// nodes of the particle's cell, then bilinear in (dx1, dx2).  Folded into one weighted sum per
-// component: along an axis where the component sits at half-integer positions the three weights are
-// {(1-d)/2, 1/2, d/2} on samples {c-1, c, c+1}; where it sits on nodes, {1-d, d} on {c, c+1}.
-// `F` is any accessor with  T operator()(int comp, int di, int dj)  returning sample
-// (i1 + di, i2 + dj) of component comp (0..5 = D1 D2 D3 B1 B2 B3).
+// corner nodes of the particle's cell, then bilinear in (dx1, dx2).
+//   node value of a component at half-integer positions along axis 1 only (D1, B2): (F(i-1,j) + F(i,j))/2
+//   along axis 2 only (D2, B1): (F(i,j-1) + F(i,j))/2;  along both (B3): mean of the four;  D3 sits on nodes.
+// `F(comp, di, dj)` returns sample (i1 + di, i2 + dj) of component comp (0..5 = D1 D2 D3 B1 B2 B3).
+// The tiled kernel does stage (i) once per tile in shared memory and calls bilinear() only.
 // ------------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ T bilinear(T c00, T c10, T c01, T c11, T dx1, T dx2) {
+  const T o1 = T(1) - dx1;
+  const T lo = fma_(c10, dx1, c00 * o1);
+  const T hi = fma_(c11, dx1, c01 * o1);
+  return fma_(hi, dx2, lo * (T(1) - dx2));
+}
+
+template <typename T, typename Acc>
+__device__ __forceinline__ T node_value(const Acc& F, int comp, int kind, int i, int j) {
+  switch (kind) {
+    case 0: return F(comp, i, j);
+    case 1: return T(0.5) * (F(comp, i - 1, j) + F(comp, i, j));
+    case 2: return T(0.5) * (F(comp, i, j - 1) + F(comp, i, j));
+    default: return T(0.25) * (((F(comp, i - 1, j - 1) + F(comp, i - 1, j)) + F(comp, i, j - 1)) + F(comp, i, j));
+  }
+}
+
+// staggering kind of each component: 1 = half-integer along x1, 2 = along x2, 3 = both, 0 = on nodes
+__device__ __forceinline__ constexpr int yee_kind(int comp) {
+  return comp == 0 ? 1 : comp == 1 ? 2 : comp == 2 ? 0 : comp == 3 ? 2 : comp == 4 ? 1 : 3;
+}
+
 template <typename T, typename Acc>
 __device__ __forceinline__ void interp_fields(const Acc& F, T dx1, T dx2, T D[3], T B[3]) {
-  const T n1[2] = {T(1) - dx1, dx1};
-  const T n2[2] = {T(1) - dx2, dx2};
-  const T h1[3] = {T(0.5) * n1[0], T(0.5), T(0.5) * dx1};
-  const T h2[3] = {T(0.5) * n2[0], T(0.5), T(0.5) * dx2};
-  T acc;
-  // D1(i+1/2, j), B2(i+1/2, j): half-integer along 1, nodes along 2
-  acc = T(0);
+  T out[6];
 #pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int l = 0; l < 2; ++l) acc = fma_(h1[k] * n2[l], F(0, k - 1, l), acc);
-  D[0] = acc;
-  acc = T(0);
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int l = 0; l < 2; ++l) acc = fma_(h1[k] * n2[l], F(4, k - 1, l), acc);
-  B[1] = acc;
-  // D2(i, j+1/2), B1(i, j+1/2): nodes along 1, half-integer along 2
-  acc = T(0);
-#pragma unroll
-  for (int k = 0; k < 2; ++k)
-#pragma unroll
-    for (int l = 0; l < 3; ++l) acc = fma_(n1[k] * h2[l], F(1, k, l - 1), acc);
-  D[1] = acc;
-  acc = T(0);
-#pragma unroll
-  for (int k = 0; k < 2; ++k)
-#pragma unroll
-    for (int l = 0; l < 3; ++l) acc = fma_(n1[k] * h2[l], F(3, k, l - 1), acc);
-  B[0] = acc;
-  // D3(i, j): nodes
-  acc = T(0);
-#pragma unroll
-  for (int k = 0; k < 2; ++k)
-#pragma unroll
-    for (int l = 0; l < 2; ++l) acc = fma_(n1[k] * n2[l], F(2, k, l), acc);
-  D[2] = acc;
-  // B3(i+1/2, j+1/2): half-integer along both
-  acc = T(0);
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int l = 0; l < 3; ++l) acc = fma_(h1[k] * h2[l], F(5, k - 1, l - 1), acc);
-  B[2] = acc;
+  for (int c = 0; c < 6; ++c) {
+    const int kind = yee_kind(c);
+    const T c00 = node_value<T>(F, c, kind, 0, 0), c10 = node_value<T>(F, c, kind, 1, 0);
+    const T c01 = node_value<T>(F, c, kind, 0, 1), c11 = node_value<T>(F, c, kind, 1, 1);
+    out[c] = bilinear(c00, c10, c01, c11, dx1, dx2);
+  }
+  D[0] = out[0]; D[1] = out[1]; D[2] = out[2];
+  B[0] = out[3]; B[1] = out[4]; B[2] = out[5];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -360,42 +445,51 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
   T u[3] = {p.u1, p.u2, p.u3};
   {
     T r, sth, cth;
-    X.at(g, T(0), T(0), r, sth, cth);
+    X.at0(g, r, sth, cth);
     MetricFull<T> m;
     metric_full(g, r, sth, cth, m);
 
     Tetrad<T> e;
-    T Dh[3], Bh[3], uh[3];
-    const T c = qm * m.alpha * dt * T(0.25);
+    T cD[3], cB[3], uh[3];
     if (em) {
+      const T c = (qm * T(0.25)) * (m.alpha * dt);
+      T Dh[3], Bh[3];
       e.init(m);
       e.cntrv_to_tetrad(Dp, Dh);                         // step 3
       e.cntrv_to_tetrad(Bp, Bh);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) { cD[k] = c * Dh[k]; cB[k] = c * Bh[k]; }
       e.cov_to_tetrad(u, uh);
-      boris_half(Dh, Bh, c, uh);                         // step 4
+      boris_half(cD, cB, uh);                            // step 4
       e.tetrad_to_cov(uh, u);                            // step 5
     }
     // step 6, Eq. 26-27: metric frozen at x^(n); exactly n_iter applications, u~(0) = u*
     {
       const T us0 = u[0], us1 = u[1], u3 = u[2];
-      // everything that does not change with the iterate (u_3 is fixed)
-      const T g2c = eps + m.hu33 * u3 * u3;
-      const T f0c = m.d_hu33[0] * u3 * u3, f1c = m.d_hu33[1] * u3 * u3;
-      const T h13u3 = T(2) * m.hu13 * u3;
-      const T d13u3_0 = T(2) * m.d_hu13[0] * u3, d13u3_1 = T(2) * m.d_hu13[1] * u3;
+      // everything that does not change with the iterate (u_3 is fixed), dt folded in
+      const T u3sq = u3 * u3;
+      const T g2c = fma_(m.hu33, u3sq, eps);
+      const T f0c = m.d_hu33[0] * u3sq, f1c = m.d_hu33[1] * u3sq;
+      const T h13u3 = (T(2) * m.hu13) * u3;
+      const T d13u3_0 = (T(2) * m.d_hu13[0]) * u3, d13u3_1 = (T(2) * m.d_hu13[1]) * u3;
+      const T dta0 = dt * m.d_alpha[0], dta1 = dt * m.d_alpha[1];
+      const T dtb0 = dt * m.d_beta1[0], dtb1 = dt * m.d_beta1[1];
+      const T hadt = (T(0.5) * m.alpha) * dt;             // dt * alpha/2, so that hadt/gamma = dt/(2 u^0)
+      const T hus0 = T(0.5) * us0, hus1 = T(0.5) * us1;
       T ut0 = us0, ut1 = us1;
       for (int it = 0; it < g.n_iter; ++it) {
-        const T ub0 = T(0.5) * (us0 + ut0), ub1 = T(0.5) * (us1 + ut1);
-        const T gam2 = g2c + ub0 * (m.hu11 * ub0 + h13u3) + m.hu22 * ub1 * ub1;
+        const T ub0 = fma_(T(0.5), ut0, hus0), ub1 = fma_(T(0.5), ut1, hus1);
+        const T ub1sq = ub1 * ub1;
+        const T gam2 = fma_(ub0, fma_(m.hu11, ub0, h13u3), fma_(m.hu22, ub1sq, g2c));
         const T igam = rsqrt_(gam2);
         const T gam = gam2 * igam;                        // alpha u^0
-        const T hiu0 = T(0.5) * m.alpha * igam;           // 1/(2 u^0)
-        const T q0 = f0c + ub0 * (m.d_hu11[0] * ub0 + d13u3_0) + m.d_hu22[0] * ub1 * ub1;
-        const T q1 = f1c + ub0 * (m.d_hu11[1] * ub0 + d13u3_1) + m.d_hu22[1] * ub1 * ub1;
-        const T nt0 = us0 + dt * (-gam * m.d_alpha[0] + ub0 * m.d_beta1[0] - hiu0 * q0);
-        const T nt1 = us1 + dt * (-gam * m.d_alpha[1] + ub0 * m.d_beta1[1] - hiu0 * q1);
+        const T hiu0 = hadt * igam;                       // dt/(2 u^0)
+        const T q0 = fma_(ub0, fma_(m.d_hu11[0], ub0, d13u3_0), fma_(m.d_hu22[0], ub1sq, f0c));
+        const T q1 = fma_(ub0, fma_(m.d_hu11[1], ub0, d13u3_1), fma_(m.d_hu22[1], ub1sq, f1c));
+        const T nt0 = fma_(-hiu0, q0, fma_(ub0, dtb0, fma_(-gam, dta0, us0)));
+        const T nt1 = fma_(-hiu0, q1, fma_(ub0, dtb1, fma_(-gam, dta1, us1)));
         // the map is deterministic: once an iterate repeats bit for bit every later one equals it
-        const bool fixed = (nt0 == ut0) && (nt1 == ut1);
+        const bool fixed = (nt0 == ut0) & (nt1 == ut1);
         ut0 = nt0;
         ut1 = nt1;
         if (fixed && g.early_exit) break;
@@ -405,25 +499,23 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
     }
     if (em) {
       e.cov_to_tetrad(u, uh);                            // step 7
-      boris_half(Dh, Bh, c, uh);                         // step 8
+      boris_half(cD, cB, uh);                            // step 8
       e.tetrad_to_cov(uh, u);                            // step 9
     }
   }
   // step 10, Eq. 28-29 in displacement space: del = x~ - x^(n); all coefficients at x^(n) + del/2
   T del1 = T(0), del2 = T(0);
-  MetricLite<T> mm;
-  T iu0 = T(0);
-  const T u1sq = u[0] * u[0], u2sq = u[1] * u[1], u3sq = u[2] * u[2], u1u3x2 = T(2) * u[0] * u[2];
+  MidU<T> U;
+  U.init(g, u[0], u[1], u[2], eps, dt);
+  MidEval<T> E;
   bool fixed = false;
   for (int it = 0; it < g.n_iter; ++it) {
     T r, sth, cth;
     X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
-    metric_lite(g, r, sth, cth, mm);
-    iu0 = inv_u0(mm, u1sq, u2sq, u3sq, u1u3x2, eps);
-    const T n1 = dt * ((mm.hu11 * u[0] + mm.hu13 * u[2]) * iu0 - mm.beta1);
-    const T n2 = dt * (mm.hu22 * u[1] * iu0);
+    T n1, n2;
+    E.eval(g, U, r, sth, n1, n2);
     // bit-identical iterate => every later iterate is the same: stopping here IS n_iter iterations
-    fixed = (n1 == del1) && (n2 == del2);
+    fixed = (n1 == del1) & (n2 == del2);
     del1 = n1;
     del2 = n2;
     if (fixed && g.early_exit) break;
@@ -431,12 +523,11 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
   // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2.  If the last iterate repeated, the midpoint
   // of the last evaluation is x_m itself and its coefficients are reused; otherwise evaluate there.
   if (!fixed) {
-    T r, sth, cth;
+    T r, sth, cth, n1, n2;
     X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
-    metric_lite(g, r, sth, cth, mm);
-    iu0 = inv_u0(mm, u1sq, u2sq, u3sq, u1u3x2, eps);
+    E.eval(g, U, r, sth, n1, n2);
   }
-  dphidt = (mm.hu13 * u[0] + mm.hu33 * u[2]) * iu0;
+  dphidt = E.dphidt(g, U);
   // renormalise to (cell, displacement in [0,1))
   T t1 = p.dx1 + del1, t2 = p.dx2 + del2;
   const T f1 = floor_(t1), f2 = floor_(t2);
@@ -466,14 +557,13 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
 // J3 = q w (alpha/gamma) u^3 (Eq. 36), half per segment, bilinear on the cell's four nodes.
 //
 // `v3` = (alpha/gamma)(h^13 u_1 + h^33 u_3) at the midpoint of the deposited path.
-// `sink(s, J1lo, J1hi, J2lo, J2hi, J3_00, J3_10, J3_01, J3_11)` receives, for segment s:
-//    J1(c1+1/2, c2) += J1lo   J1(c1+1/2, c2+1) += J1hi
-//    J2(c1, c2+1/2) += J2lo   J2(c1+1, c2+1/2) += J2hi
-//    J3(c1+k, c2+l) += J3_kl
+// seg[s][0..7] receives, for segment s with cell (c1, c2):
+//    [0] J1(c1+1/2, c2)   [1] J1(c1+1/2, c2+1)   [2] J2(c1, c2+1/2)   [3] J2(c1+1, c2+1/2)
+//    [4] J3(c1, c2)       [5] J3(c1+1, c2)       [6] J3(c1, c2+1)     [7] J3(c1+1, c2+1)
 // ------------------------------------------------------------------------------------------------
-template <typename T, typename Sink>
+template <typename T>
 __device__ __forceinline__ void deposit_segments(int di, int dj, T xa, T ya, T dx1_new, T dx2_new, T qw_over_dt,
-                                                 T qw, T v3, Sink&& sink) {
+                                                 T qw, T v3, T seg[2][8]) {
   const T xb = (T)di + dx1_new, yb = (T)dj + dx2_new;
   const T xr = fmin((T)(di < 0 ? di : 0) + T(1), fmax((T)(di > 0 ? di : 0), T(0.5) * (xa + xb)));
   const T yr = fmin((T)(dj < 0 ? dj : 0) + T(1), fmax((T)(dj > 0 ? dj : 0), T(0.5) * (ya + yb)));
@@ -482,30 +572,36 @@ __device__ __forceinline__ void deposit_segments(int di, int dj, T xa, T ya, T d
     const T F1 = qw_over_dt * (xr - xa), F2 = qw_over_dt * (yr - ya);
     const T W1 = T(0.5) * (xa + xr), W2 = T(0.5) * (ya + yr);
     const T F3a = F3 * (T(1) - W1), F3b = F3 * W1;
-    sink(0, F1 * (T(1) - W2), F1 * W2, F2 * (T(1) - W1), F2 * W1, F3a * (T(1) - W2), F3b * (T(1) - W2), F3a * W2,
-         F3b * W2);
+    seg[0][0] = F1 * (T(1) - W2); seg[0][1] = F1 * W2;
+    seg[0][2] = F2 * (T(1) - W1); seg[0][3] = F2 * W1;
+    seg[0][4] = F3a * (T(1) - W2); seg[0][5] = F3b * (T(1) - W2);
+    seg[0][6] = F3a * W2; seg[0][7] = F3b * W2;
   }
   {
     const T F1 = qw_over_dt * (xb - xr), F2 = qw_over_dt * (yb - yr);
     const T W1 = T(0.5) * (xr + xb) - (T)di, W2 = T(0.5) * (yr + yb) - (T)dj;
     const T F3a = F3 * (T(1) - W1), F3b = F3 * W1;
-    sink(1, F1 * (T(1) - W2), F1 * W2, F2 * (T(1) - W1), F2 * W1, F3a * (T(1) - W2), F3b * (T(1) - W2), F3a * W2,
-         F3b * W2);
+    seg[1][0] = F1 * (T(1) - W2); seg[1][1] = F1 * W2;
+    seg[1][2] = F2 * (T(1) - W1); seg[1][3] = F2 * W1;
+    seg[1][4] = F3a * (T(1) - W2); seg[1][5] = F3b * (T(1) - W2);
+    seg[1][6] = F3a * W2; seg[1][7] = F3b * W2;
   }
 }
 
-// out-of-plane velocity of Eq. 36 at the midpoint of the path (ia + (xa+xb)/2, ja + (ya+yb)/2), theta clamped
+// out-of-plane velocity of Eq. 36 at the midpoint of the path (ia + xm, ja + ym), theta clamped
 template <typename T>
 __device__ __forceinline__ T v3_at_path_midpoint(const Consts<T>& g, int ia, int ja, T xm, T ym, T u1, T u2, T u3,
                                                  T eps) {
   Coord<T> X;
   X.init(g, ia, xm, ja, ym);
   T r, sth, cth;
-  X.at(g, T(0), T(0), r, sth, cth);
-  MetricLite<T> mm;
-  metric_lite(g, r, sth, cth, mm);
-  const T iu0 = inv_u0(mm, u1 * u1, u2 * u2, u3 * u3, T(2) * u1 * u3, eps);
-  return (mm.hu13 * u1 + mm.hu33 * u3) * iu0;
+  X.at0(g, r, sth, cth);
+  MidU<T> U;
+  U.init(g, u1, u2, u3, eps, T(1));
+  MidEval<T> E;
+  T n1, n2;
+  E.eval(g, U, r, sth, n1, n2);
+  return E.dphidt(g, U);
 }
 
 }  // namespace grpic

@@ -72,23 +72,18 @@ struct GlobalFieldAcc {
 __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
 __device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
 
+// eight additions of one deposit segment (layout of deposit_segments' seg[s][0..7]) at cell offset k
 template <typename T>
-struct GlobalJSink {
-  const JPtrs<T>& J;
-  int64_t o[2];  // offsets of cells (ia,ja), (ib,jb)
-  int ld;
-  __device__ __forceinline__ void operator()(int s, T a0, T a1, T b0, T b1, T c00, T c10, T c01, T c11) const {
-    const int64_t k = o[s];
-    red_add(J.j[0] + k, a0);
-    red_add(J.j[0] + k + 1, a1);
-    red_add(J.j[1] + k, b0);
-    red_add(J.j[1] + k + ld, b1);
-    red_add(J.j[2] + k, c00);
-    red_add(J.j[2] + k + ld, c10);
-    red_add(J.j[2] + k + 1, c01);
-    red_add(J.j[2] + k + ld + 1, c11);
-  }
-};
+__device__ __forceinline__ void global_add8(const JPtrs<T>& J, int64_t k, int ld, const T v[8]) {
+  red_add(J.j[0] + k, v[0]);
+  red_add(J.j[0] + k + 1, v[1]);
+  red_add(J.j[1] + k, v[2]);
+  red_add(J.j[1] + k + ld, v[3]);
+  red_add(J.j[2] + k, v[4]);
+  red_add(J.j[2] + k + ld, v[5]);
+  red_add(J.j[2] + k + 1, v[6]);
+  red_add(J.j[2] + k + ld + 1, v[7]);
+}
 
 // ------------------------------------------------------------------------------------------------
 // shared per-particle driver used by k_push / k_step_direct
@@ -135,8 +130,16 @@ __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<
           v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
                                    p.u2, p.u3, eps);
         const T qw = (T)sc.charge * P.w[k];
-        GlobalJSink<T> sink{J, {cell, cell + (int64_t)di * g.ld + dj}, g.ld};
-        deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw / dt, qw, v3, sink);
+        T seg[2][8];
+        deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw / dt, qw, v3, seg);
+        if (di == 0 && dj == 0) {                          // both segments in one cell: one set of additions
+#pragma unroll
+          for (int q = 0; q < 8; ++q) seg[0][q] += seg[1][q];
+          global_add8(J, cell, g.ld, seg[0]);
+        } else {
+          global_add8(J, cell, g.ld, seg[0]);
+          global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
+        }
       }
     }
   }
@@ -174,8 +177,10 @@ __global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPt
                                        P.u2[k], P.u3[k], eps);
       const T qw = (T)sc.charge * P.w[k];
       const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
-      GlobalJSink<T> sink{J, {cell, cell + (int64_t)di * g.ld + dj}, g.ld};
-      deposit_segments(di, dj, xa, ya, dx1, dx2, qw / (T)sc.dt, qw, v3, sink);
+      T seg[2][8];
+      deposit_segments(di, dj, xa, ya, dx1, dx2, qw / (T)sc.dt, qw, v3, seg);
+      global_add8(J, cell, g.ld, seg[0]);
+      global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
     }
   }
   warp_count(counters, 3, over);

@@ -4,14 +4,19 @@
 //   1. one elected thread issues six 2-D TMA loads (cp.async.bulk.tensor) that bring the tile's
 //      field stencil — (kTile + 2 kHalo + 2) x (kTile + 2 kHalo + 6) samples of each of D1 D2 D3 B1 B2 B3 — into shared
 //      memory, completion tracked by an mbarrier; out-of-range rows/columns are zero-filled by TMA;
-//   2. every thread pushes its particles (steps 1-11 + BCs) with the gather served from shared
-//      memory; a particle that has drifted out of the window since the last sort falls back to
-//      global gathers, so the result never depends on how stale the table is;
-//   3. J is accumulated in a shared-memory tile: contributions of lanes that deposit into the same
-//      cell are first summed across the warp (segmented shuffle reduction over runs of equal cell),
-//      then one lane per run issues the shared atomics; particles leaving the window use global
-//      reductions;
-//   4. one flush of the non-zero shared J entries to HBM with red.global.add.
+//   2. stage (i) of the gather (R-S4) is done ONCE per tile: the six Yee components are averaged to the
+//      (kTile + 2 kHalo + 1)^2 nodes of the window and stored node-major (8 reals per node), so that a
+//      particle's gather is four 32/64-byte node reads and six bilinear forms;
+//   3. every thread pushes its particles (steps 1-11 + BCs); a particle that has drifted out of the
+//      window since the last sort falls back to global gathers, so the result never depends on how
+//      stale the table is;
+//   4. J is accumulated in a shared-memory tile.  Shared FP atomics are compare-and-swap loops on
+//      sm_100a (LDS + FADD + ATOMS.CAST.SPIN + BRA, retried on every address collision), so the
+//      contributions are first summed across the warp: lanes depositing into the same cell form a
+//      group; the group's eight values are reduced with a transposing butterfly (9 shuffles instead of
+//      40) that leaves each of the eight sums in a different lane, and those eight lanes issue ONE
+//      conflict-free shared atomic.  Particles leaving the window use global reductions;
+//   5. one flush of the non-zero shared J entries to HBM with red.global.add.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -89,20 +94,22 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
       : "memory");
 }
 
-// ---- shared-memory accessors ----
+// ---- shared-memory layout ----
+constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
+constexpr int kNodeStride = 8;                  // reals per node: D1 D2 D3 B1 B2 B3 + 2 pad (128-bit reads)
+constexpr int kJStride = kWinF;                 // row stride of the shared J tile
+constexpr int kJComp = kWinJ * kJStride;        // one component
+constexpr int kRawElems = 6 * kWinF * kRowF;    // staged raw stencil; reused as the J tile after stage (i)
+constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride;
+static_assert(3 * kJComp <= kRawElems, "the J tile must fit into the raw staging buffer it aliases");
+
 template <typename T>
-struct SmemFieldAcc {
-  const T* base;  // sample (c1, c2) of component 0, i.e. the particle's own cell
-  __device__ __forceinline__ T operator()(int c, int di, int dj) const {
-    return base[c * (kWinF * kRowF) + di * kRowF + dj];
-  }
-};
+constexpr size_t tiled_smem_bytes() {
+  return (size_t)(kRawElems + kNodeElems) * sizeof(T) + 16;
+}
 
 __device__ __forceinline__ void smem_add(float* p, float v) { atomicAdd(p, v); }
 __device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }
-
-constexpr int kJStride = kWinF;                 // row stride of the shared J tile
-constexpr int kJComp = kWinJ * kJStride;        // one component
 
 template <typename T>
 __device__ __forceinline__ void smem_add8(T* sJ, int node, const T v[8]) {
@@ -116,52 +123,98 @@ __device__ __forceinline__ void smem_add8(T* sJ, int node, const T v[8]) {
   smem_add(sJ + 2 * kJComp + node + kJStride + 1, v[7]);
 }
 
-template <typename T>
-__device__ __forceinline__ void global_add8(const JPtrs<T>& J, int64_t k, int ld, const T v[8]) {
-  red_add(J.j[0] + k, v[0]);
-  red_add(J.j[0] + k + 1, v[1]);
-  red_add(J.j[1] + k, v[2]);
-  red_add(J.j[1] + k + ld, v[3]);
-  red_add(J.j[2] + k, v[4]);
-  red_add(J.j[2] + k + ld, v[5]);
-  red_add(J.j[2] + k + 1, v[6]);
-  red_add(J.j[2] + k + ld + 1, v[7]);
+// offset inside the shared J tile of value q (0..7, layout of deposit_segments) relative to the cell's node
+__device__ __forceinline__ int j_offset_of(int q) {
+  const int comp = (q < 2) ? 0 : ((q < 4) ? 1 : 2);
+  const int d1 = (q == 3 || q == 5 || q == 7) ? kJStride : 0;
+  const int d2 = (q == 1 || q == 6 || q == 7) ? 1 : 0;
+  return comp * kJComp + d1 + d2;
 }
 
-// Warp-aggregated flush of the per-lane run accumulators into the shared J tile: lanes holding the same
-// cell key in consecutive lanes form a run; the run is summed with log2(32) shuffle steps and its first
-// lane issues the eight shared atomics.  (Shared FP atomics are compare-and-swap loops on sm_100a —
-// ATOMS.CAST.SPIN — so fewer, conflict-free atomics is what matters.)
 template <typename T>
-__device__ __forceinline__ void warp_flush_runs(T* sJ, int lane, bool valid, int node, T acc[8]) {
-  const int key = valid ? node : (0x40000000 + lane);                 // idle lanes: unique keys
-  const int key_prev = __shfl_up_sync(0xffffffffu, key, 1);
-  const bool head = (lane == 0) || (key != key_prev);
-  const unsigned heads = __ballot_sync(0xffffffffu, head);
-  const unsigned above = heads & ~((2u << lane) - 1u);                // run heads strictly above my lane
-  const int run_last = above ? (__ffs(above) - 2) : 31;               // last lane of my run
+__device__ __forceinline__ T shfl_xor_(T v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+
+// Warp-aggregated addition into the shared J tile.  Lanes with `has` hold a cell `key` (node index in the
+// tile) and eight values.  Lanes with equal key form a group; per group the eight values are summed over
+// the group's lanes by a transposing butterfly: after the xor-16 step a lane keeps four of the eight
+// partial sums, after xor-8 two, after xor-4 one, then two plain steps — 9 shuffles, and the sum of value
+// q = 4*bit4 + 2*bit3 + bit2 ends in the lanes with those bits; the eight lanes with (lane & 3) == 0 add
+// them to eight different addresses in one shared atomic instruction.  At most kMaxPass groups are
+// handled this way per call (cell-sorted particles give 1-3 groups per warp); lanes left over add alone.
+constexpr int kMaxPass = 4;
+
+template <typename T>
+__device__ __forceinline__ void warp_group_add(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
+  unsigned pending = __ballot_sync(0xffffffffu, has);
+  for (int pass = 0; pass < kMaxPass && pending; ++pass) {
+    const int leader = __ffs(pending) - 1;
+    const int k0 = __shfl_sync(0xffffffffu, key, leader);
+    const bool mine = has && key == k0;
+    pending &= ~__ballot_sync(0xffffffffu, mine);
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+    T x[4], y[2], z;
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const bool take = (lane + d) <= run_last;
+    for (int j = 0; j < 4; ++j) {
+      const T lo = mine ? v[j] : T(0), hi = mine ? v[j + 4] : T(0);
+      x[j] = (b4 ? hi : lo) + shfl_xor_(b4 ? lo : hi, 16);
+    }
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-      const T o = __shfl_down_sync(0xffffffffu, acc[q], d);
-      if (take) acc[q] += o;
+    for (int j = 0; j < 2; ++j) y[j] = (b3 ? x[j + 2] : x[j]) + shfl_xor_(b3 ? x[j] : x[j + 2], 8);
+    z = (b2 ? y[1] : y[0]) + shfl_xor_(b2 ? y[0] : y[1], 4);
+    z += shfl_xor_(z, 2);
+    z += shfl_xor_(z, 1);
+    if ((lane & 3) == 0 && z != T(0)) smem_add(sJ + k0 + my_off, z);
+  }
+  if (pending) {
+    if (has && ((pending >> lane) & 1u)) smem_add8(sJ, key, v);
+  }
+}
+
+// node-major shared field accessor: four node reads, six bilinear forms
+template <typename T>
+__device__ __forceinline__ void interp_nodes(const T* nod, int n00, T dx1, T dx2, T D[3], T B[3]) {
+  T c[4][kNodeStride];
+  const int idx[4] = {n00, n00 + kNodeW, n00 + 1, n00 + kNodeW + 1};   // (0,0) (1,0) (0,1) (1,1)
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    if (sizeof(T) == 4) {
+      const float4* p = reinterpret_cast<const float4*>(nod + idx[k] * kNodeStride);
+      const float4 a = p[0], b = p[1];
+      c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)a.z; c[k][3] = (T)a.w; c[k][4] = (T)b.x; c[k][5] = (T)b.y;
+    } else {
+      const double2* p = reinterpret_cast<const double2*>(nod + idx[k] * kNodeStride);
+      const double2 a = p[0], b = p[1], d = p[2];
+      c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)b.x; c[k][3] = (T)b.y; c[k][4] = (T)d.x; c[k][5] = (T)d.y;
     }
   }
-  if (head && valid) smem_add8(sJ, node, acc);
+  D[0] = bilinear(c[0][0], c[1][0], c[2][0], c[3][0], dx1, dx2);
+  D[1] = bilinear(c[0][1], c[1][1], c[2][1], c[3][1], dx1, dx2);
+  D[2] = bilinear(c[0][2], c[1][2], c[2][2], c[3][2], dx1, dx2);
+  B[0] = bilinear(c[0][3], c[1][3], c[2][3], c[3][3], dx1, dx2);
+  B[1] = bilinear(c[0][4], c[1][4], c[2][4], c[3][4], dx1, dx2);
+  B[2] = bilinear(c[0][5], c[1][5], c[2][5], c[3][5], dx1, dx2);
 }
 
 template <typename T>
-__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
-                                                       const JPtrs<T> J, const SpeciesConst sc,
-                                                       unsigned long long* counters, const WorkItem* items,
-                                                       const uint32_t* n_items_ptr, uint32_t max_items,
-                                                       int64_t n_at_sort, int nt2, int use_tma,
-                                                       const __grid_constant__ FieldMaps maps) {
-  __shared__ __align__(128) T sF[6 * kWinF * kRowF];
-  __shared__ __align__(16) T sJ[3 * kJComp];
-  __shared__ __align__(8) uint64_t bar;
+struct RawAcc {      // raw staged stencil: sample (row, col) of component c
+  const T* raw;
+  int row, col;
+  __device__ __forceinline__ T operator()(int c, int di, int dj) const {
+    return raw[c * (kWinF * kRowF) + (row + di) * kRowF + (col + dj)];
+  }
+};
+
+template <typename T>
+__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
+    k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
+                 unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
+                 uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma,
+                 const __grid_constant__ FieldMaps maps) {
+  extern __shared__ __align__(128) unsigned char smem_raw_[];
+  T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the J tile
+  T* sN = sF + kRawElems;                             // node-major averaged fields
+  T* sJ = sF;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sN + kNodeElems);
 
   const int tid = threadIdx.x, lane = tid & 31;
   // ---- tail blocks: particles appended after the last sort -> direct path ----
@@ -182,54 +235,57 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled
   // ---- 1. stage the field stencil ----
   if (use_tma) {
     if (tid == 0) {
-      mbar_init(&bar, 1);
+      mbar_init(bar, 1);
       mbar_fence_init();
     }
     __syncthreads();
     if (tid == 0) {
-      mbar_expect_tx(&bar, 6u * kWinF * kRowF * (uint32_t)sizeof(T));
+      mbar_expect_tx(bar, 6u * kWinF * kRowF * (uint32_t)sizeof(T));
 #pragma unroll
       for (int c = 0; c < 6; ++c)
-        tma_load_2d(sF + c * kWinF * kRowF, &maps.m[c], a2lo - off2, c1lo - 1 + g.ng, &bar);
+        tma_load_2d(sF + c * kWinF * kRowF, &maps.m[c], a2lo - off2, c1lo - 1 + g.ng, bar);
     }
+    mbar_wait(bar, 0);
   } else {
     const int rows = g.n1 + 2 * g.ng;
-    for (int e = tid; e < 6 * kWinF * kRowF; e += kBlock) {
+    for (int e = tid; e < kRawElems; e += kBlock) {
       const int c = e / (kWinF * kRowF), rem = e % (kWinF * kRowF);
       const int a1 = c1lo - 1 + g.ng + rem / kRowF, a2 = a2lo - off2 + rem % kRowF;
       sF[e] = (a1 >= 0 && a1 < rows && a2 >= 0 && a2 < g.ld) ? __ldg(F.f[c] + (int64_t)a1 * g.ld + a2) : T(0);
     }
+    __syncthreads();
   }
-  for (int e = tid; e < 3 * kJComp; e += kBlock) sJ[e] = T(0);
+  // ---- 2. stage (i) of the gather: Yee samples -> nodes (R-S4), node-major ----
+  for (int n = tid; n < kNodeW * kNodeW; n += kBlock) {
+    const int w1 = n / kNodeW, w2 = n % kNodeW;
+    const RawAcc<T> acc{sF, w1 + 1, w2 + 1 + off2};
+    T* o = sN + n * kNodeStride;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) o[c] = node_value<T>(acc, c, yee_kind(c), 0, 0);
+    o[6] = T(0); o[7] = T(0);
+  }
   __syncthreads();
-  if (use_tma) mbar_wait(&bar, 0);
+  for (int e = tid; e < 3 * kJComp; e += kBlock) sJ[e] = T(0);   // the raw stencil is dead: it becomes the J tile
+  __syncthreads();
 
-  // ---- 2./3. particles ----
+  // ---- 3./4. particles ----
   const T eps = sc.massive ? T(1) : T(0);
   const T dt = (T)sc.dt;
   const T inv_dt = T(1) / dt;
+  const int my_off = j_offset_of(((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1));
   const uint32_t end = item.begin + item.count;
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
-  // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): different warps then work on
-  // different cells, and consecutive iterations of one lane stay in the same cell, so contributions
-  // are first accumulated per lane in registers (acc) and flushed only when some lane changes cell.
+  // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): the 32 particles of one iteration
+  // then sit in one to three cells, which is what makes the warp-level aggregation cheap.
   const uint32_t per_warp = ((item.count + kBlock - 1) / kBlock) * 32u;
   const uint32_t w_begin = item.begin + (uint32_t)(tid >> 5) * per_warp;
   const uint32_t w_end = min(end, w_begin + per_warp);
-  bool acc_valid = false;
-  int acc_node = 0;
-  T acc[8];
-#pragma unroll
-  for (int q = 0; q < 8; ++q) acc[q] = T(0);
   for (uint32_t base = w_begin; base < w_end; base += 32u) {
     const uint32_t k = base + lane;
     const bool alive = k < w_end && P.tag[k] != 0;
-    int res = -1;
-    bool dep_smem = false, dep_cross = false;
-    int node_a = 0x7fffffff, node_b = 0;
-    T va[8], vb[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) va[q] = vb[q] = T(0);
+    bool dep_a = false, dep_b = false;
+    int node_a = 0, node_b = 0;
+    T seg[2][8];
     if (alive) {
       PState<T> p;
       p.i1 = P.i1[k]; p.i2 = P.i2[k];
@@ -243,15 +299,14 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled
       const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
       T Dp[3], Bp[3];
       if (a_in) {
-        SmemFieldAcc<T> acc{sF + (wa1 + 1) * kRowF + (wa2 + 1 + off2)};
-        interp_fields(acc, p.dx1, p.dx2, Dp, Bp);
+        interp_nodes(sN, wa1 * kNodeW + wa2, p.dx1, p.dx2, Dp, Bp);
       } else {
         GlobalFieldAcc<T> acc{F, cell, g.ld};
         interp_fields(acc, p.dx1, p.dx2, Dp, Bp);
       }
       T dphidt;
       bool reflected;
-      res = push_particle(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
+      const int res = push_particle(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
       P.i1[k] = p.i1; P.i2[k] = p.i2; P.dx1[k] = p.dx1; P.dx2[k] = p.dx2;
       P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
       if (sc.has_phi) P.phi[k] += dt * dphidt;
@@ -266,51 +321,30 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled
             v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
                                      p.u2, p.u3, eps);
           const T qw = (T)sc.charge * P.w[k];
-          T seg[2][8];
-          deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw * inv_dt, qw, v3,
-                           [&seg](int s, T a0, T a1, T b0, T b1, T c00, T c10, T c01, T c11) {
-                             seg[s][0] = a0; seg[s][1] = a1; seg[s][2] = b0; seg[s][3] = b1;
-                             seg[s][4] = c00; seg[s][5] = c10; seg[s][6] = c01; seg[s][7] = c11;
-                           });
+          deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw * inv_dt, qw, v3, seg);
           const int wb1 = wa1 + di, wb2 = wa2 + dj;
           const bool b_in = (unsigned)wb1 < (unsigned)kWinC && (unsigned)wb2 < (unsigned)kWinC;
+          const bool cross = (di != 0) || (dj != 0);
+          if (!cross) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) seg[0][q] += seg[1][q];
+          }
           if (a_in && b_in) {
-            dep_smem = true;
+            dep_a = true;
+            dep_b = cross;
             node_a = wa1 * kJStride + wa2;
-            if (di == 0 && dj == 0) {
-#pragma unroll
-              for (int q = 0; q < 8; ++q) va[q] = seg[0][q] + seg[1][q];
-            } else {
-              dep_cross = true;
-              node_b = wb1 * kJStride + wb2;
-#pragma unroll
-              for (int q = 0; q < 8; ++q) { va[q] = seg[0][q]; vb[q] = seg[1][q]; }
-            }
+            node_b = wb1 * kJStride + wb2;
           } else {
             global_add8(J, cell, g.ld, seg[0]);
-            global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
+            if (cross) global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
           }
         }
       }
       n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
     }
-    // ---- run accumulation: flush (warp-aggregated) when any lane leaves its cell ----
-    const bool must_flush = acc_valid && (!dep_smem || node_a != acc_node);
-    if (__any_sync(0xffffffffu, must_flush)) {
-      warp_flush_runs(sJ, lane, acc_valid, acc_node, acc);
-      acc_valid = false;
-#pragma unroll
-      for (int q = 0; q < 8; ++q) acc[q] = T(0);
-    }
-    if (dep_smem) {
-      acc_valid = true;
-      acc_node = node_a;
-#pragma unroll
-      for (int q = 0; q < 8; ++q) acc[q] += va[q];
-      if (dep_cross) smem_add8(sJ, node_b, vb);
-    }
+    warp_group_add(sJ, lane, my_off, dep_a, node_a, seg[0]);
+    if (__any_sync(0xffffffffu, dep_b)) warp_group_add(sJ, lane, my_off, dep_b, node_b, seg[1]);
   }
-  if (__any_sync(0xffffffffu, acc_valid)) warp_flush_runs(sJ, lane, acc_valid, acc_node, acc);
   // counters: one atomic per warp and counter
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -326,7 +360,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1)) k_step_tiled
     if (n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
     if (n_alive + n_in + n_out) atomicAdd(&counters[4], (unsigned long long)(n_alive + n_in + n_out));
   }
-  // ---- 4. flush ----
+  // ---- 5. flush ----
   __syncthreads();
   const int rows = g.n1 + 2 * g.ng;
   for (int e = tid; e < 3 * kJComp; e += kBlock) {
@@ -344,6 +378,16 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
                        const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
                        cudaStream_t st, std::string& err) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)tiled_smem_bytes<T>());
+    if (ea != cudaSuccess) {
+      err = std::string("k_step_tiled shared-memory opt-in: ") + cudaGetErrorString(ea);
+      return false;
+    }
+    attr_set = true;
+  }
   FieldMaps maps;
   memset(&maps, 0, sizeof(maps));
   int use_tma = want_tma ? 1 : 0;
@@ -353,8 +397,8 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   const int nt2 = (g.n2 + kTile - 1) / kTile;
   const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
   const unsigned grid = max_items + (unsigned)((tail + kBlock - 1) / kBlock);
-  k_step_tiled<T><<<grid, kBlock, 0, st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items, n_at_sort, nt2,
-                                           use_tma, maps);
+  k_step_tiled<T><<<grid, kBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
+                                                                n_at_sort, nt2, use_tma, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     err = std::string("k_step_tiled launch: ") + cudaGetErrorString(e);
