@@ -10,13 +10,14 @@
 //   3. every thread pushes its particles (steps 1-11 + BCs); a particle that has drifted out of the
 //      window since the last sort falls back to global gathers, so the result never depends on how
 //      stale the table is;
-//   4. J is accumulated in a shared-memory tile.  Shared FP atomics are compare-and-swap loops on
-//      sm_100a (LDS + FADD + ATOMS.CAST.SPIN + BRA, retried on every address collision), so the
-//      contributions are first summed across the warp: lanes depositing into the same cell form a
-//      group; the group's eight values are reduced with a transposing butterfly (9 shuffles instead of
-//      40) that leaves each of the eight sums in a different lane, and those eight lanes issue ONE
-//      conflict-free shared atomic.  Particles leaving the window use global reductions;
-//   5. one flush of the non-zero shared J entries to HBM with red.global.add.
+//   4. J is accumulated in shared memory, one PRIVATE tile per warp.  Shared FP atomics are
+//      compare-and-swap loops on sm_100a (LDS + FADD + ATOMS.CAST.SPIN + BRA, retried on every address
+//      collision); with a tile per warp none is needed: lanes depositing into the same cell are
+//      summed across the warp first (transposing butterfly, 9 shuffles instead of 40, for groups of
+//      kBigGroup or more lanes; rank-by-rank rounds for the small groups), and what is left are plain
+//      read-modify-writes whose lanes never share an address.  Particles leaving the window use
+//      global reductions;
+//   5. one flush: the private tiles are summed and the non-zero entries go to HBM with red.global.add.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -97,33 +98,22 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
 // ---- shared-memory layout ----
 constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
 constexpr int kNodeStride = 8;                  // reals per node: D1 D2 D3 B1 B2 B3 + 2 pad (128-bit reads)
-constexpr int kJStride = kWinF;                 // row stride of the shared J tile
+constexpr int kJStride = kWinF;                 // row stride of one shared J tile
 constexpr int kJComp = kWinJ * kJStride;        // one component
-constexpr int kRawElems = 6 * kWinF * kRowF;    // staged raw stencil; reused as the J tile after stage (i)
+constexpr int kJTile = 3 * kJComp;              // one private J tile (J1 J2 J3)
+constexpr int kWarps = kBlock / 32;
+constexpr int kRawElems = 6 * kWinF * kRowF;    // staged raw stencil; its space is reused by the J tiles after stage (i)
+constexpr int kJElems = kWarps * kJTile;        // one PRIVATE J tile per warp: no atomics inside the CTA
+constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
 constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride;
-static_assert(3 * kJComp <= kRawElems, "the J tile must fit into the raw staging buffer it aliases");
+static_assert(kJTile % 4 == 0 && kFrontElems % 4 == 0, "128-bit zero fill");
 
 template <typename T>
 constexpr size_t tiled_smem_bytes() {
-  return (size_t)(kRawElems + kNodeElems) * sizeof(T) + 16;
+  return (size_t)(kFrontElems + kNodeElems) * sizeof(T) + 16;
 }
 
-__device__ __forceinline__ void smem_add(float* p, float v) { atomicAdd(p, v); }
-__device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }
-
-template <typename T>
-__device__ __forceinline__ void smem_add8(T* sJ, int node, const T v[8]) {
-  smem_add(sJ + node, v[0]);
-  smem_add(sJ + node + 1, v[1]);
-  smem_add(sJ + kJComp + node, v[2]);
-  smem_add(sJ + kJComp + node + kJStride, v[3]);
-  smem_add(sJ + 2 * kJComp + node, v[4]);
-  smem_add(sJ + 2 * kJComp + node + kJStride, v[5]);
-  smem_add(sJ + 2 * kJComp + node + 1, v[6]);
-  smem_add(sJ + 2 * kJComp + node + kJStride + 1, v[7]);
-}
-
-// offset inside the shared J tile of value q (0..7, layout of deposit_segments) relative to the cell's node
+// offset inside a shared J tile of value q (0..7, layout of deposit_segments) relative to the cell's node
 __device__ __forceinline__ int j_offset_of(int q) {
   const int comp = (q < 2) ? 0 : ((q < 4) ? 1 : 2);
   const int d1 = (q == 3 || q == 5 || q == 7) ? kJStride : 0;
@@ -134,39 +124,84 @@ __device__ __forceinline__ int j_offset_of(int q) {
 template <typename T>
 __device__ __forceinline__ T shfl_xor_(T v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 
-// Warp-aggregated addition into the shared J tile.  Lanes with `has` hold a cell `key` (node index in the
-// tile) and eight values.  Lanes with equal key form a group; per group the eight values are summed over
-// the group's lanes by a transposing butterfly: after the xor-16 step a lane keeps four of the eight
-// partial sums, after xor-8 two, after xor-4 one, then two plain steps — 9 shuffles, and the sum of value
-// q = 4*bit4 + 2*bit3 + bit2 ends in the lanes with those bits; the eight lanes with (lane & 3) == 0 add
-// them to eight different addresses in one shared atomic instruction.  At most kMaxPass groups are
-// handled this way per call (cell-sorted particles give 1-3 groups per warp); lanes left over add alone.
-constexpr int kMaxPass = 4;
+// Eight plain read-modify-writes of one deposit segment into the warp's PRIVATE J tile, for all lanes
+// with `on` at once.  Precondition: the lanes with `on` hold pairwise different cells (`node`).  Then the
+// lanes of one instruction never share an address; addresses shared between DIFFERENT values of
+// neighbouring cells (J1(c,c2+1) of cell c2 = J1(c,c2) of cell c2+1, ...) are kept apart by the four
+// phases, each closed by __syncwarp() (memory ordering among the lanes of the warp).
+template <typename T>
+__device__ __forceinline__ void private_add8(T* sJ, bool on, int node, const T v[8]) {
+  if (on) {
+    sJ[node] += v[0];
+    sJ[kJComp + node] += v[2];
+    sJ[2 * kJComp + node] += v[4];
+  }
+  __syncwarp();
+  if (on) {
+    sJ[node + 1] += v[1];
+    sJ[kJComp + node + kJStride] += v[3];
+    sJ[2 * kJComp + node + kJStride] += v[5];
+  }
+  __syncwarp();
+  if (on) sJ[2 * kJComp + node + 1] += v[6];
+  __syncwarp();
+  if (on) sJ[2 * kJComp + node + kJStride + 1] += v[7];
+  __syncwarp();
+}
+
+// Warp-aggregated addition into the warp's private J tile.  Lanes with `has` hold a cell `key` (node index
+// in the tile) and eight values.  __match_any_sync groups the lanes by cell.
+//   - A group of kBigGroup or more lanes (cell-sorted particles: usually the whole warp) is summed by a
+//     transposing butterfly: after the xor-16 step a lane keeps four of the eight partial sums, after
+//     xor-8 two, after xor-4 one, then two plain steps — 9 shuffles, and the sum of value
+//     q = 4*bit4 + 2*bit3 + bit2 ends in the lanes with those bits; the eight lanes with (lane & 3) == 0
+//     add them to eight different addresses with ONE plain read-modify-write.
+//   - The lanes of smaller groups are served by rank inside their group: round r takes the r-th lane of
+//     every group, so the lanes of one round hold pairwise different cells (private_add8).
+constexpr int kBigGroup = 4;
 
 template <typename T>
-__device__ __forceinline__ void warp_group_add(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
-  unsigned pending = __ballot_sync(0xffffffffu, has);
-  for (int pass = 0; pass < kMaxPass && pending; ++pass) {
-    const int leader = __ffs(pending) - 1;
+__device__ __forceinline__ void warp_deposit(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
+  const unsigned act = __ballot_sync(0xffffffffu, has);
+  if (act == 0u) return;
+  const unsigned peers = __match_any_sync(0xffffffffu, has ? key : ~lane);
+  const int cnt = __popc(peers);
+  unsigned big = __ballot_sync(0xffffffffu, has && cnt >= kBigGroup);
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+  while (big) {
+    const int leader = __ffs(big) - 1;
+    const unsigned pm = __shfl_sync(0xffffffffu, peers, leader);
     const int k0 = __shfl_sync(0xffffffffu, key, leader);
-    const bool mine = has && key == k0;
-    pending &= ~__ballot_sync(0xffffffffu, mine);
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+    big &= ~pm;
     T x[4], y[2], z;
+    if (pm == 0xffffffffu) {                       // the whole warp deposits into one cell: no masking
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const T lo = mine ? v[j] : T(0), hi = mine ? v[j + 4] : T(0);
-      x[j] = (b4 ? hi : lo) + shfl_xor_(b4 ? lo : hi, 16);
+      for (int j = 0; j < 4; ++j) x[j] = (b4 ? v[j + 4] : v[j]) + shfl_xor_(b4 ? v[j] : v[j + 4], 16);
+    } else {
+      const bool mine = (pm >> lane) & 1u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const T lo = mine ? v[j] : T(0), hi = mine ? v[j + 4] : T(0);
+        x[j] = (b4 ? hi : lo) + shfl_xor_(b4 ? lo : hi, 16);
+      }
     }
 #pragma unroll
     for (int j = 0; j < 2; ++j) y[j] = (b3 ? x[j + 2] : x[j]) + shfl_xor_(b3 ? x[j] : x[j + 2], 8);
     z = (b2 ? y[1] : y[0]) + shfl_xor_(b2 ? y[0] : y[1], 4);
     z += shfl_xor_(z, 2);
     z += shfl_xor_(z, 1);
-    if ((lane & 3) == 0 && z != T(0)) smem_add(sJ + k0 + my_off, z);
+    if ((lane & 3) == 0) sJ[k0 + my_off] += z;
+    __syncwarp();
   }
-  if (pending) {
-    if (has && ((pending >> lane) & 1u)) smem_add8(sJ, key, v);
+  const bool small = has && cnt < kBigGroup;
+  unsigned rem = __ballot_sync(0xffffffffu, small);
+  if (rem) {
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    for (int r = 0; r < kBigGroup - 1 && rem; ++r) {
+      const bool on = small && rank == r;
+      private_add8(sJ, on, key, v);
+      rem &= ~__ballot_sync(0xffffffffu, on);
+    }
   }
 }
 
@@ -211,12 +246,12 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
                  uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma,
                  const __grid_constant__ FieldMaps maps) {
   extern __shared__ __align__(128) unsigned char smem_raw_[];
-  T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the J tile
-  T* sN = sF + kRawElems;                             // node-major averaged fields
-  T* sJ = sF;
+  T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the kWarps private J tiles
+  T* sN = sF + kFrontElems;                           // node-major averaged fields
   uint64_t* bar = reinterpret_cast<uint64_t*>(sN + kNodeElems);
 
-  const int tid = threadIdx.x, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  T* sJ = sF + wid * kJTile;                          // this warp's private J tile
   // ---- tail blocks: particles appended after the last sort -> direct path ----
   if (blockIdx.x >= max_items) {
     const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kBlock + tid;
@@ -265,32 +300,46 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
     o[6] = T(0); o[7] = T(0);
   }
   __syncthreads();
-  for (int e = tid; e < 3 * kJComp; e += kBlock) sJ[e] = T(0);   // the raw stencil is dead: it becomes the J tile
+  {                                                    // the raw stencil is dead: its space becomes the J tiles
+    float4* z4 = reinterpret_cast<float4*>(sF);
+    constexpr int n4 = (int)(kJElems * sizeof(T) / 16);
+    for (int e = tid; e < n4; e += kBlock) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   __syncthreads();
 
   // ---- 3./4. particles ----
   const T eps = sc.massive ? T(1) : T(0);
   const T dt = (T)sc.dt;
   const T inv_dt = T(1) / dt;
+  const T chg = (T)sc.charge;
   const int my_off = j_offset_of(((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1));
   const uint32_t end = item.begin + item.count;
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
   // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): the 32 particles of one iteration
   // then sit in one to three cells, which is what makes the warp-level aggregation cheap.
   const uint32_t per_warp = ((item.count + kBlock - 1) / kBlock) * 32u;
-  const uint32_t w_begin = item.begin + (uint32_t)(tid >> 5) * per_warp;
+  const uint32_t w_begin = item.begin + (uint32_t)wid * per_warp;
   const uint32_t w_end = min(end, w_begin + per_warp);
   for (uint32_t base = w_begin; base < w_end; base += 32u) {
     const uint32_t k = base + lane;
-    const bool alive = k < w_end && P.tag[k] != 0;
+    const bool in = k < w_end;
+    // all columns are requested at once (one exposed memory latency per iteration, not three)
+    PState<T> p;
+    T w = T(0), phi = T(0);
+    uint8_t tg = 0;
+    if (in) {
+      tg = P.tag[k];
+      p.i1 = P.i1[k]; p.i2 = P.i2[k];
+      p.dx1 = P.dx1[k]; p.dx2 = P.dx2[k];
+      p.u1 = P.u1[k]; p.u2 = P.u2[k]; p.u3 = P.u3[k];
+      w = P.w[k];
+      if (sc.has_phi) phi = P.phi[k];
+    }
+    const bool alive = in && tg != 0;
     bool dep_a = false, dep_b = false;
     int node_a = 0, node_b = 0;
     T seg[2][8];
     if (alive) {
-      PState<T> p;
-      p.i1 = P.i1[k]; p.i2 = P.i2[k];
-      p.dx1 = P.dx1[k]; p.dx2 = P.dx2[k];
-      p.u1 = P.u1[k]; p.u2 = P.u2[k]; p.u3 = P.u3[k];
       const int ia = p.i1, ja = p.i2;
       const T xa = p.dx1, ya = p.dx2;
       P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya;
@@ -309,7 +358,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
       const int res = push_particle(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
       P.i1[k] = p.i1; P.i2[k] = p.i2; P.dx1[k] = p.dx1; P.dx2[k] = p.dx2;
       P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
-      if (sc.has_phi) P.phi[k] += dt * dphidt;
+      if (sc.has_phi) P.phi[k] = phi + dt * dphidt;
       if (res != 0) P.tag[k] = 0;
       if (res == 0) {
         const int di = p.i1 - ia, dj = p.i2 - ja;
@@ -320,7 +369,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
           if (reflected)
             v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
                                      p.u2, p.u3, eps);
-          const T qw = (T)sc.charge * P.w[k];
+          const T qw = chg * w;
           deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw * inv_dt, qw, v3, seg);
           const int wb1 = wa1 + di, wb2 = wa2 + dj;
           const bool b_in = (unsigned)wb1 < (unsigned)kWinC && (unsigned)wb2 < (unsigned)kWinC;
@@ -342,8 +391,8 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
       }
       n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
     }
-    warp_group_add(sJ, lane, my_off, dep_a, node_a, seg[0]);
-    if (__any_sync(0xffffffffu, dep_b)) warp_group_add(sJ, lane, my_off, dep_b, node_b, seg[1]);
+    warp_deposit(sJ, lane, my_off, dep_a, node_a, seg[0]);
+    warp_deposit(sJ, lane, my_off, dep_b, node_b, seg[1]);
   }
   // counters: one atomic per warp and counter
 #pragma unroll
@@ -360,11 +409,13 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
     if (n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
     if (n_alive + n_in + n_out) atomicAdd(&counters[4], (unsigned long long)(n_alive + n_in + n_out));
   }
-  // ---- 5. flush ----
+  // ---- 5. flush: sum the private tiles, one reduction per touched entry ----
   __syncthreads();
   const int rows = g.n1 + 2 * g.ng;
-  for (int e = tid; e < 3 * kJComp; e += kBlock) {
-    const T v = sJ[e];
+  for (int e = tid; e < kJTile; e += kBlock) {
+    T v = sF[e];
+#pragma unroll
+    for (int q = 1; q < kWarps; ++q) v += sF[q * kJTile + e];
     if (v != T(0)) {
       const int c = e / kJComp, rem = e % kJComp;
       const int a1 = c1lo + g.ng + rem / kJStride, a2 = c2lo + g.ng + rem % kJStride;
