@@ -42,7 +42,8 @@ def build(force: bool = False, verbose: bool = False) -> dict:
         so = lib_path(prec)
         out[prec] = so
         if force or _stale(so):
-            cmd = [nvcc] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + \
+            extra = os.environ.get("GRPIC_NVCC_EXTRA", "").split()      # e.g. "-DGRPIC_TILED_MINB=2" for tuning runs
+            cmd = [nvcc] + NVCC_FLAGS + defs + extra + (["-Xptxas", "-v"] if verbose else []) + \
                   [os.path.join(_CSRC, "grpic.cu"), "-o", so]
             procs.append((prec, cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for prec, cmd, p in procs:

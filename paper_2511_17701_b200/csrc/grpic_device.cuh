@@ -69,6 +69,24 @@ __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a
 __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
 __device__ __forceinline__ float below_one(float) { return 0x1.fffffep-1f; }
 
+// A kernel parameter copied into a register the compiler cannot rematerialise from the constant bank:
+// without this ptxas re-reads loop constants with LDCU + MOV in every iteration of the fixed-point loops.
+__device__ __forceinline__ float in_reg(float x) {
+  float y;
+  asm volatile("mov.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double in_reg(double x) {
+  double y;
+  asm volatile("mov.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return y;
+}
+__device__ __forceinline__ int in_reg(int x) {
+  int y;
+  asm volatile("mov.s32 %0, %1;" : "=r"(y) : "r"(x));
+  return y;
+}
+
 // exp(e) - 1 ... as 1 + e + ... and sin(d), cos(d) for the small in-step displacements of the midpoint
 // iteration.  Truncation errors (relative): FP32 |e| < 0.04: e^5/120 < 1e-9; |d| < 0.045: d^4/120, d^6/720 < 4e-8.
 // FP64 |e| < 0.04: e^11/11! < 2e-23; |d| < 0.045: d^12/12!, d^13/13! < 2e-25.
@@ -161,6 +179,29 @@ struct Coord<double> {
     if (th < g.th_min) { sth = g.sin_min; cth = g.cos_min; }
     if (th > g.th_max) { sth = g.sin_max; cth = g.cos_max; }
   }
+  // Loop form of at(): r and sin(theta) only (Eq. 29 needs no cos), polynomial branch only, loop constants
+  // in registers.  Returns false if the displacement is outside SmallLimits (the caller then redoes the
+  // loop with at()).  Same arithmetic as the polynomial branch of at().
+  struct Fast {
+    double hdxi, deta, th_min, th_max, sin_min, sin_max;
+    __device__ __forceinline__ void init(const Consts<double>& g, const Coord<double>&) {
+      hdxi = in_reg(0.5 * g.dxi); deta = in_reg(g.deta);
+      th_min = in_reg(g.th_min); th_max = in_reg(g.th_max);
+      sin_min = in_reg(g.sin_min); sin_max = in_reg(g.sin_max);
+    }
+  };
+  __device__ __forceinline__ bool at_fast(const Fast& f, double del1, double del2, double& r, double& sth) const {
+    const double e = del1 * f.hdxi;
+    const double th = (x2 + 0.5 * del2) * f.deta;
+    const double d = th - th0;
+    r = r0 * exp_small(e);
+    double sd, cd;
+    sincos_small(d, sd, cd);
+    sth = fma(s0, cd, c0 * sd);
+    if (th < f.th_min) sth = f.sin_min;
+    if (th > f.th_max) sth = f.sin_max;
+    return fabs(e) < SmallLimits<double>::e && fabs(d) < SmallLimits<double>::d;
+  }
 };
 
 template <>
@@ -206,6 +247,27 @@ struct Coord<float> {
     sth = s;
     cth = sgn * c;
   }
+  // Loop form of at(): r and sin(theta) only, polynomial branch only, loop constants in registers.
+  // theta' = thp + d is measured from the nearer axis, so inside SmallLimits it never reaches th_max and
+  // only the lower clamp is tested.  Returns false outside SmallLimits (the caller redoes the loop with at()).
+  struct Fast {
+    float hdxi, hdeta, th_min, sin_min;
+    __device__ __forceinline__ void init(const Consts<float>& g, const Coord<float>& X) {
+      hdxi = in_reg(0.5f * g.dxi); hdeta = in_reg((0.5f * X.sgn) * g.deta);
+      th_min = in_reg(g.th_min); sin_min = in_reg(g.sin_min);
+    }
+  };
+  __device__ __forceinline__ bool at_fast(const Fast& f, float del1, float del2, float& r, float& sth) const {
+    const float e = del1 * f.hdxi;
+    const float d = del2 * f.hdeta;
+    r = r0 * exp_small(e);
+    float sd, cd;
+    sincos_small(d, sd, cd);
+    float s = fmaf(s0, cd, c0 * sd);
+    if (thp + d < f.th_min) s = f.sin_min;
+    sth = s;
+    return fabsf(e) < SmallLimits<float>::e && fabsf(d) < SmallLimits<float>::d;
+  }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -223,7 +285,7 @@ struct MidU {           // per-particle constants of the coordinate loop
   T U2sq;               // (u_2/deta)^2
   T u3, u3sq, au3, c2au3;
   T k1, k2;             // dt/dxi,  dt u_2/deta^2
-  T eps;
+  T eps, a2;
   __device__ __forceinline__ void init(const Consts<T>& g, T u1, T u2, T u3_, T eps_, T dt) {
     w1c = u1 * g.inv_dxi;
     U2sq = (u2 * u2) * g.inv_deta2;
@@ -234,6 +296,7 @@ struct MidU {           // per-particle constants of the coordinate loop
     k1 = dt * g.inv_dxi;
     k2 = (dt * u2) * g.inv_deta2;
     eps = eps_;
+    a2 = in_reg(g.a2);
   }
 };
 
@@ -242,16 +305,16 @@ struct MidEval {
   T R, w1, is2;
   // returns the two displacement rates times dt
   __device__ __forceinline__ void eval(const Consts<T>& g, const MidU<T>& U, T r, T sth, T& n1, T& n2) {
-    const T r2 = r * r;
-    const T a2s2 = g.a2 * (sth * sth);
-    const T r2a2 = r2 + g.a2;
+    const T s2 = sth * sth;
+    const T a2s2 = U.a2 * s2;
+    const T r2a2 = fma_(r, r, U.a2);
     const T Sigma = r2a2 - a2s2;
     const T Sp2r = fma_(T(2), r, Sigma);
-    const T Delta = fma_(r, r - T(2), g.a2);
+    const T Delta = fma_(r, r - T(2), U.a2);
     const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
     const T ir = rcp_(r);
     const T iSp2r = rcp_(Sp2r);
-    is2 = rcp_(sth * sth);
+    is2 = rcp_(s2);
     w1 = U.w1c * ir;
     const T t = (A * iSp2r) * w1;
     T G = fma_(U.eps, Sigma, U.U2sq);
@@ -477,7 +540,9 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
       const T hadt = (T(0.5) * m.alpha) * dt;             // dt * alpha/2, so that hadt/gamma = dt/(2 u^0)
       const T hus0 = T(0.5) * us0, hus1 = T(0.5) * us1;
       T ut0 = us0, ut1 = us1;
-      for (int it = 0; it < g.n_iter; ++it) {
+      const int n_iter_u = in_reg(g.n_iter);
+      const bool ee_u = g.early_exit != 0;
+      for (int it = 0; it < n_iter_u; ++it) {
         const T ub0 = fma_(T(0.5), ut0, hus0), ub1 = fma_(T(0.5), ut1, hus1);
         const T ub1sq = ub1 * ub1;
         const T gam2 = fma_(ub0, fma_(m.hu11, ub0, h13u3), fma_(m.hu22, ub1sq, g2c));
@@ -492,7 +557,7 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
         const bool fixed = (nt0 == ut0) & (nt1 == ut1);
         ut0 = nt0;
         ut1 = nt1;
-        if (fixed && g.early_exit) break;
+        if (fixed && ee_u) break;
       }
       u[0] = ut0;
       u[1] = ut1;
@@ -509,23 +574,44 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
   U.init(g, u[0], u[1], u[2], eps, dt);
   MidEval<T> E;
   bool fixed = false;
-  for (int it = 0; it < g.n_iter; ++it) {
-    T r, sth, cth;
-    X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
-    T n1, n2;
-    E.eval(g, U, r, sth, n1, n2);
-    // bit-identical iterate => every later iterate is the same: stopping here IS n_iter iterations
-    fixed = (n1 == del1) & (n2 == del2);
-    del1 = n1;
-    del2 = n2;
-    if (fixed && g.early_exit) break;
-  }
-  // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2.  If the last iterate repeated, the midpoint
-  // of the last evaluation is x_m itself and its coefficients are reused; otherwise evaluate there.
-  if (!fixed) {
-    T r, sth, cth, n1, n2;
-    X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
-    E.eval(g, U, r, sth, n1, n2);
+  {
+    // fast form: polynomial coordinates, loop constants pinned in registers, no branch but the exit test
+    typename Coord<T>::Fast XF;
+    XF.init(g, X);
+    const int n_iter = in_reg(g.n_iter);
+    const bool ee = g.early_exit != 0;
+    bool ok = true;
+    for (int it = 0; it < n_iter; ++it) {
+      T r, sth, n1, n2;
+      ok &= X.at_fast(XF, del1, del2, r, sth);
+      E.eval(g, U, r, sth, n1, n2);
+      // bit-identical iterate => every later iterate is the same: stopping here IS n_iter iterations
+      fixed = (n1 == del1) & (n2 == del2);
+      del1 = n1;
+      del2 = n2;
+      if (fixed && ee) break;
+    }
+    // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2.  If the last iterate repeated, the midpoint
+    // of the last evaluation is x_m itself and its coefficients are reused; otherwise evaluate there.
+    if (ok && !fixed) {
+      T r, sth, n1, n2;
+      ok &= X.at_fast(XF, del1, del2, r, sth);
+      E.eval(g, U, r, sth, n1, n2);
+    }
+    if (!ok) {
+      // a displacement left SmallLimits (many cells in one step): redo the loop with the library functions
+      del1 = T(0); del2 = T(0);
+      for (int it = 0; it < g.n_iter; ++it) {
+        T r, sth, cth, n1, n2;
+        X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
+        E.eval(g, U, r, sth, n1, n2);
+        del1 = n1;
+        del2 = n2;
+      }
+      T r, sth, cth, n1, n2;
+      X.at(g, T(0.5) * del1, T(0.5) * del2, r, sth, cth);
+      E.eval(g, U, r, sth, n1, n2);
+    }
   }
   dphidt = E.dphidt(g, U);
   // renormalise to (cell, displacement in [0,1))

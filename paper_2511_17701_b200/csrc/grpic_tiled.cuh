@@ -230,6 +230,10 @@ __device__ __forceinline__ void interp_nodes(const T* nod, int n00, T dx1, T dx2
   B[2] = bilinear(c[0][5], c[1][5], c[2][5], c[3][5], dx1, dx2);
 }
 
+#ifndef GRPIC_TILED_MINB
+#define GRPIC_TILED_MINB 2      // resident CTAs per SM the FP32 tiled kernel is compiled for (128 registers: no spills, room for the prefetch)
+#endif
+
 template <typename T>
 struct RawAcc {      // raw staged stencil: sample (row, col) of component c
   const T* raw;
@@ -240,7 +244,7 @@ struct RawAcc {      // raw staged stencil: sample (row, col) of component c
 };
 
 template <typename T>
-__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
+__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
                  uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma,
@@ -320,21 +324,34 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? 3 : 1))
   const uint32_t per_warp = ((item.count + kBlock - 1) / kBlock) * 32u;
   const uint32_t w_begin = item.begin + (uint32_t)wid * per_warp;
   const uint32_t w_end = min(end, w_begin + per_warp);
+  // Software pipeline: the columns of the NEXT 32 particles are requested before the current 32 are
+  // pushed, so that their HBM latency is covered by ~1500 instructions of arithmetic.
+  struct Cols {
+    PState<T> p;
+    T w, phi;
+    uint8_t tg;
+  };
+  auto fetch = [&](uint32_t kk, bool ok, Cols& c) {
+    c.tg = 0; c.w = T(0); c.phi = T(0);
+    c.p.i1 = 0; c.p.i2 = 0; c.p.dx1 = c.p.dx2 = c.p.u1 = c.p.u2 = c.p.u3 = T(0);
+    if (ok) {
+      c.tg = P.tag[kk];
+      c.p.i1 = P.i1[kk]; c.p.i2 = P.i2[kk];
+      c.p.dx1 = P.dx1[kk]; c.p.dx2 = P.dx2[kk];
+      c.p.u1 = P.u1[kk]; c.p.u2 = P.u2[kk]; c.p.u3 = P.u3[kk];
+      c.w = P.w[kk];
+      if (sc.has_phi) c.phi = P.phi[kk];
+    }
+  };
+  Cols nxt;
+  fetch(w_begin + lane, w_begin + lane < w_end, nxt);
   for (uint32_t base = w_begin; base < w_end; base += 32u) {
     const uint32_t k = base + lane;
     const bool in = k < w_end;
-    // all columns are requested at once (one exposed memory latency per iteration, not three)
-    PState<T> p;
-    T w = T(0), phi = T(0);
-    uint8_t tg = 0;
-    if (in) {
-      tg = P.tag[k];
-      p.i1 = P.i1[k]; p.i2 = P.i2[k];
-      p.dx1 = P.dx1[k]; p.dx2 = P.dx2[k];
-      p.u1 = P.u1[k]; p.u2 = P.u2[k]; p.u3 = P.u3[k];
-      w = P.w[k];
-      if (sc.has_phi) phi = P.phi[k];
-    }
+    PState<T> p = nxt.p;
+    const T w = nxt.w, phi = nxt.phi;
+    const uint8_t tg = nxt.tg;
+    fetch(k + 32u, k + 32u < w_end, nxt);
     const bool alive = in && tg != 0;
     bool dep_a = false, dep_b = false;
     int node_a = 0, node_b = 0;
