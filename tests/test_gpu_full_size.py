@@ -1,0 +1,166 @@
+"""Full-size GPU checks (pytest -m gpu): BASELINE.json's configs at their real sizes, in the launch
+configuration bench.py times (grpic_sort, then the fused tiled grpic_step), checked on sampled particles
+the oracle recomputes one by one and on properties that hold at any size (discrete continuity Eq. 32/34,
+first moments, conserved u_3 and energy of geodesics)."""
+import numpy as np
+import pytest
+
+from helpers import TOL, compare_particles, grid_from_domain, oracle_from_cols
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def G():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2511_17701_b200 import grpic
+    grpic.load("f32"); grpic.load("f64")
+    return grpic
+
+
+def _gather(ps, idx):
+    return {k: (None if v is None else v[idx].cpu().numpy().copy()) for k, v in ps.cols.items()}
+
+
+def _cic_rho(torch, shape, ng, i1, i2, dx1, dx2, qw, mask):
+    """rho~ on nodes with the linear shape (the definition Eq. 32/34 is written for), FP64 on the device."""
+    ld = shape[1]
+    rho = torch.zeros(shape[0] * shape[1], dtype=torch.float64, device=i1.device)
+    base = (i1.long() + ng) * ld + (i2.long() + ng)
+    x, y = dx1.double(), dx2.double()
+    q = torch.where(mask, qw.double(), torch.zeros_like(x))
+    for a, wx in ((0, 1 - x), (1, x)):
+        for b, wy in ((0, 1 - y), (1, y)):
+            rho.index_add_(0, base + a * ld + b, q * wx * wy)
+    return rho.view(shape)
+
+
+def test_config4_large_full_size(G, O, W):
+    """Config 4 at full size (2048x1024, 134M particles, FP32): sort + tiled fused step as bench.py runs it.
+    (a) 2^17 sampled particles per species (plus the ragged ends of the sorted order) against the oracle;
+    (b) counters add up; (c) discrete continuity of the deposited J with the particles' own (prev -> new)
+    positions at every node; (d) first moments of J."""
+    import torch
+    wl = W.config_large()
+    dom = wl.dom
+    g = grid_from_domain(O, dom)
+    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision="f32")
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    fdev = G.grid_tensors(wl.fields, names, "f32")
+    fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
+    Jtot = {k: torch.zeros(ctx.shape, dtype=torch.float64, device="cuda") for k in ("J1", "J2", "J3")}
+    J = {k: torch.zeros(ctx.shape, dtype=torch.float32, device="cuda") for k in ("J1", "J2", "J3")}
+    rng = np.random.default_rng(44)
+    rho_diff = torch.zeros(ctx.shape, dtype=torch.float64, device="cuda")
+    m1 = m2 = 0.0
+    scale = 0.0
+    for sp in wl.species:
+        ps = G.ParticleSet.from_host(sp, "f32")
+        n = ps.n
+        ctx.sort(ps)
+        ctx.step(ps, fdev, J, wl.dt)            # one step to leave the freshly sorted state (drifted particles)
+        for v in J.values():
+            v.zero_()
+        idx_np = np.unique(np.concatenate([rng.integers(0, n, 1 << 17), np.arange(0, 4096), np.arange(n - 4096, n)]))
+        idx = torch.from_numpy(idx_np).cuda()
+        before = _gather(ps, idx)
+        ctx.step(ps, fdev, J, wl.dt)
+        c = ctx.counters()
+        for k in J:
+            Jtot[k] += J[k].double()
+        scale = max(scale, float(J["J1"].abs().max()), float(J["J2"].abs().max()))   # largest one-species |J| entry
+        after = _gather(ps, idx)
+        # (a) sampled particles, one by one in the oracle
+        op = oracle_from_cols(O, before, ps.q_over_m, ps.charge, ps.massive)
+        diag = {}
+        O.push(g, op, fhost, wl.dt, diag=diag)
+        res = compare_particles(op, after, "f32", before["tag"], g.n1, g.n2, diag=diag)
+        print("config4 full", sp.name, res, c)
+        # (b) counters
+        alive_after = int(ps.cols["tag"].sum())
+        assert c["alive"] == alive_after and c["overstep"] == 0
+        assert c["alive"] + c["absorbed_in"] + c["absorbed_out"] <= n
+        # (c), (d) accumulate continuity terms of this species: particles alive after the step deposited
+        m = ps.cols["tag"] != 0
+        qw = ps.cols["weight"] * ps.charge
+        rho_new = _cic_rho(torch, ctx.shape, dom.ng, ps.cols["i1"], ps.cols["i2"], ps.cols["dx1"], ps.cols["dx2"], qw, m)
+        rho_old = _cic_rho(torch, ctx.shape, dom.ng, ps.cols["i1_prev"], ps.cols["i2_prev"], ps.cols["dx1_prev"],
+                           ps.cols["dx2_prev"], qw, m)
+        rho_diff += rho_new - rho_old
+        d1 = (ps.cols["i1"] - ps.cols["i1_prev"]).double() + (ps.cols["dx1"].double() - ps.cols["dx1_prev"].double())
+        d2 = (ps.cols["i2"] - ps.cols["i2_prev"]).double() + (ps.cols["dx2"].double() - ps.cols["dx2_prev"].double())
+        q64 = torch.where(m, qw.double(), torch.zeros_like(d1))
+        m1 += float((q64 * d1).sum()) / wl.dt
+        m2 += float((q64 * d2).sum()) / wl.dt
+        scale_sp = float(q64.abs().sum()) / wl.dt
+        del ps, rho_new, rho_old, d1, d2, q64
+        torch.cuda.empty_cache()
+    J1, J2 = Jtot["J1"], Jtot["J2"]
+    div = torch.zeros_like(J1)
+    div[1:, :] += J1[1:, :] - J1[:-1, :]
+    div[:, 1:] += J2[:, 1:] - J2[:, :-1]
+    resid = rho_diff / wl.dt + div
+    # scale: the largest one-species |J| entry; FP32 sums of a few hundred contributions per entry -> ~1e-6 relative
+    r = float(resid[1:, 1:].abs().max()) / scale
+    print("config4 full: continuity residual / max|J| =", r)
+    assert r < 5e-6
+    # first moments: sum over the grid of J^i = sum_p q w dx^i/dt   (species of opposite charge cancel in the
+    # total, so compare against the per-species magnitude scale)
+    e1 = abs(float(J1.sum()) - m1) / scale_sp
+    e2 = abs(float(J2.sum()) - m2) / scale_sp
+    print("config4 full: first-moment errors", e1, e2)
+    assert e1 < 1e-6 and e2 < 1e-6
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_config2_geodesic_full_size_100_steps(G, O, W, prec):
+    """Config 2 at full size: 2^24 zero-charge particles, a = 0.95, 100 steps of dt = 0.01.
+    Sampled particles against the oracle at the first and the last step; u_3 bit-identical after 100 steps
+    (Eq. 27: u~_3 = u_3); the circular-orbit half keeps its radius (fixed points of Eq. 28-29) and the
+    conserved energy -u_0 = alpha*gamma - beta^1 u_1 of every surviving geodesic stays within the
+    integrator's second-order error."""
+    import torch
+    from helpers import energy_u0
+    wl = W.config_geodesic(n=1 << 24, dtype=prec)
+    dom = wl.dom
+    g = grid_from_domain(O, dom)
+    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
+    ps = G.ParticleSet.from_host(wl.species[0], prec)
+    n = ps.n
+    u3_0 = ps.cols["u3"].clone()
+    rng = np.random.default_rng(22)
+    idx_np = np.unique(np.concatenate([rng.integers(0, n, 1 << 16), np.arange(0, 1024), np.arange(n - 1024, n)]))
+    idx = torch.from_numpy(idx_np).cuda()
+    s0 = _gather(ps, idx)
+    E0 = energy_u0(O, g, s0["i1"] + s0["dx1"].astype(np.float64), s0["i2"] + s0["dx2"].astype(np.float64),
+                   s0["u1"].astype(np.float64), s0["u2"].astype(np.float64), s0["u3"].astype(np.float64))
+    for step in range(wl.steps):
+        check = step in (0, wl.steps - 1)
+        if check:
+            before = _gather(ps, idx)
+        ctx.step(ps, None, None, wl.dt)
+        if check:
+            after = _gather(ps, idx)
+            op = oracle_from_cols(O, before, 0.0, 0.0, 1)
+            diag = {}
+            O.push(g, op, None, wl.dt, diag=diag)
+            res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag)
+            print("config2 full", prec, "step", step, res)
+    assert torch.equal(ps.cols["u3"], u3_0), "u_3 must be untouched by 100 geodesic steps"
+    s1 = _gather(ps, idx)
+    alive = s1["tag"] != 0
+    assert alive.sum() > 0.4 * len(idx_np)            # the circular half survives
+    E1 = energy_u0(O, g, s1["i1"] + s1["dx1"].astype(np.float64), s1["i2"] + s1["dx2"].astype(np.float64),
+                   s1["u1"].astype(np.float64), s1["u2"].astype(np.float64), s1["u3"].astype(np.float64))
+    dE = np.abs(E1 / E0 - 1.0)[alive]
+    # plungers close to the horizon have large second-order errors at dt = 0.01; the bound is on the bulk
+    tol_E = 1e-4
+    print("config2 full", prec, "energy drift: median", np.median(dE), "99%", np.quantile(dE, 0.99), "max", dE.max())
+    assert np.quantile(dE, 0.99) < tol_E and dE.max() < 5e-4
+    # circular orbits (first half of the arrays) stay at their radius: |dr/r| small after t = 1
+    circ = idx_np < n // 2
+    x1_0 = s0["i1"] + s0["dx1"].astype(np.float64); x1_1 = s1["i1"] + s1["dx1"].astype(np.float64)
+    drift = np.abs(x1_1 - x1_0)[circ & alive]
+    print("config2 full", prec, "circular-orbit radial drift (cells): max", drift.max())
+    assert drift.max() < 0.05
