@@ -33,10 +33,24 @@ UNIT = "updates/s"
 
 # Algorithmic figures per particle update: what the method, as the paper states
 # it with n_iter = 10, must compute and move.
-FLOPS_PER_UPDATE_NITER10 = 1972.0          # +,-,*,/,sqrt,exp,sin,cos,floor,min,max each count 1
+FLOPS_PER_UPDATE_NITER10 = 2051.0          # DESIGN.md section 7 table: +,-,*,/,sqrt,exp,sin,cos,floor,min,max,compare each count 1
 BYTES_PER_UPDATE = {"f32": 70.0, "f64": 122.0}   # fused step: read i,dx,u,phi,w,tag; write i,dx,u,phi,tag
 # FP32 FMA peak from unit counts and clocks (B200_PROFILING.md: 148 SMs, 1965 MHz; 128 FP32 lanes/SM, FMA = 2)
 ALU_PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+
+
+def _ncu_traffic(prec, workload):
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture
+    (profiles/ncu_traffic.csv: kernel,precision,workload,particles,dram_read_bytes,dram_write_bytes,source)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for line in f:
+                t = line.strip().split(",")
+                if len(t) >= 7 and t[1] == prec and t[2] == workload:
+                    return {"bytes": float(t[4]) + float(t[5]), "particles": float(t[3]), "kernel": t[0], "source": t[6]}
+    except Exception:
+        pass
+    return None
 
 
 def _peaks():
@@ -302,6 +316,7 @@ def run_ours(args):
     alu_peak = ALU_PEAK_TFLOPS[prec]
     hbm_ach = BYTES_PER_UPDATE[prec] * upd_per_launch / sec_per_launch / 1e9
     kernel = "k_step_tiled" if not args.no_tile else "k_push_or_step<.,true>"
+    tr = _ncu_traffic(prec, args.workload) if (not args.no_tile and args.shrink == 1) else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -311,7 +326,9 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "paper_context": "paper: ~1.2-1.4e8 updates/s on 1x A100 (P:550), other hardware, not a target"},
         "roofline": {"bound": "alu", "kernel": kernel, "achieved": ach_tflops, "peak": alu_peak, "unit": "TFLOP/s",
-                     "frac": ach_tflops / alu_peak, "traffic": None,
+                     "frac": ach_tflops / alu_peak, "traffic": (tr["bytes"] if tr else None),
+                     "traffic_note": (f"dram read+write bytes of one {tr['kernel']} launch over {tr['particles']:.0f} particles, "
+                                      f"{tr['source']}" if tr else None),
                      "peak_source": f"derived: 148 SMs x {128 if prec == 'f32' else 64} lanes x 2 (FMA) x 1.965 GHz",
                      "flops_per_update": FLOPS_PER_UPDATE_NITER10,
                      "updates_per_launch": upd_per_launch, "ms_per_launch": sec_per_launch * 1e3,
@@ -325,7 +342,7 @@ def run_ours(args):
     if e2e is not None:
         out["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.workload, shrink=4, steps=4)
+        out["cpu_baseline"] = cpu_baseline(args.workload, shrink=4, steps=16)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -334,7 +351,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="large")

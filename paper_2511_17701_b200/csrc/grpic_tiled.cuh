@@ -95,13 +95,22 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
       : "memory");
 }
 
+// ---- launch shape of the tiled kernel ----
+#ifndef GRPIC_TILED_BLOCK
+#define GRPIC_TILED_BLOCK 128   // threads per CTA
+#endif
+#ifndef GRPIC_TILED_MINB
+#define GRPIC_TILED_MINB 4      // resident CTAs per SM the FP32 kernel is compiled for (128 registers: no spills, room for the prefetch)
+#endif
+constexpr int kTBlock = GRPIC_TILED_BLOCK;
+
 // ---- shared-memory layout ----
 constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
 constexpr int kNodeStride = 8;                  // reals per node: D1 D2 D3 B1 B2 B3 + 2 pad (128-bit reads)
 constexpr int kJStride = kWinF;                 // row stride of one shared J tile
 constexpr int kJComp = kWinJ * kJStride;        // one component
 constexpr int kJTile = 3 * kJComp;              // one private J tile (J1 J2 J3)
-constexpr int kWarps = kBlock / 32;
+constexpr int kWarps = kTBlock / 32;
 constexpr int kRawElems = 6 * kWinF * kRowF;    // staged raw stencil; its space is reused by the J tiles after stage (i)
 constexpr int kJElems = kWarps * kJTile;        // one PRIVATE J tile per warp: no atomics inside the CTA
 constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
@@ -230,10 +239,6 @@ __device__ __forceinline__ void interp_nodes(const T* nod, int n00, T dx1, T dx2
   B[2] = bilinear(c[0][5], c[1][5], c[2][5], c[3][5], dx1, dx2);
 }
 
-#ifndef GRPIC_TILED_MINB
-#define GRPIC_TILED_MINB 2      // resident CTAs per SM the FP32 tiled kernel is compiled for (128 registers: no spills, room for the prefetch)
-#endif
-
 template <typename T>
 struct RawAcc {      // raw staged stencil: sample (row, col) of component c
   const T* raw;
@@ -244,7 +249,7 @@ struct RawAcc {      // raw staged stencil: sample (row, col) of component c
 };
 
 template <typename T>
-__global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
+__global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
                  uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma,
@@ -258,7 +263,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
   T* sJ = sF + wid * kJTile;                          // this warp's private J tile
   // ---- tail blocks: particles appended after the last sort -> direct path ----
   if (blockIdx.x >= max_items) {
-    const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kBlock + tid;
+    const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
     particle_direct<T, true>(g, P, F, J, sc, counters, k);
     return;
   }
@@ -287,7 +292,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
     mbar_wait(bar, 0);
   } else {
     const int rows = g.n1 + 2 * g.ng;
-    for (int e = tid; e < kRawElems; e += kBlock) {
+    for (int e = tid; e < kRawElems; e += kTBlock) {
       const int c = e / (kWinF * kRowF), rem = e % (kWinF * kRowF);
       const int a1 = c1lo - 1 + g.ng + rem / kRowF, a2 = a2lo - off2 + rem % kRowF;
       sF[e] = (a1 >= 0 && a1 < rows && a2 >= 0 && a2 < g.ld) ? __ldg(F.f[c] + (int64_t)a1 * g.ld + a2) : T(0);
@@ -295,7 +300,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
     __syncthreads();
   }
   // ---- 2. stage (i) of the gather: Yee samples -> nodes (R-S4), node-major ----
-  for (int n = tid; n < kNodeW * kNodeW; n += kBlock) {
+  for (int n = tid; n < kNodeW * kNodeW; n += kTBlock) {
     const int w1 = n / kNodeW, w2 = n % kNodeW;
     const RawAcc<T> acc{sF, w1 + 1, w2 + 1 + off2};
     T* o = sN + n * kNodeStride;
@@ -307,7 +312,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
   {                                                    // the raw stencil is dead: its space becomes the J tiles
     float4* z4 = reinterpret_cast<float4*>(sF);
     constexpr int n4 = (int)(kJElems * sizeof(T) / 16);
-    for (int e = tid; e < n4; e += kBlock) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int e = tid; e < n4; e += kTBlock) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
   __syncthreads();
 
@@ -321,7 +326,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
   // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): the 32 particles of one iteration
   // then sit in one to three cells, which is what makes the warp-level aggregation cheap.
-  const uint32_t per_warp = ((item.count + kBlock - 1) / kBlock) * 32u;
+  const uint32_t per_warp = ((item.count + kTBlock - 1) / kTBlock) * 32u;
   const uint32_t w_begin = item.begin + (uint32_t)wid * per_warp;
   const uint32_t w_end = min(end, w_begin + per_warp);
   // Software pipeline: the columns of the NEXT 32 particles are requested before the current 32 are
@@ -429,7 +434,7 @@ __global__ void __launch_bounds__(kBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1
   // ---- 5. flush: sum the private tiles, one reduction per touched entry ----
   __syncthreads();
   const int rows = g.n1 + 2 * g.ng;
-  for (int e = tid; e < kJTile; e += kBlock) {
+  for (int e = tid; e < kJTile; e += kTBlock) {
     T v = sF[e];
 #pragma unroll
     for (int q = 1; q < kWarps; ++q) v += sF[q * kJTile + e];
@@ -464,8 +469,8 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
     if (!enc.encode(&maps.m[c], F.f[c], (int)sizeof(T), rows, g.ld)) use_tma = 0;
   const int nt2 = (g.n2 + kTile - 1) / kTile;
   const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
-  const unsigned grid = max_items + (unsigned)((tail + kBlock - 1) / kBlock);
-  k_step_tiled<T><<<grid, kBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
+  const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
+  k_step_tiled<T><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
                                                                 n_at_sort, nt2, use_tma, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
