@@ -147,6 +147,20 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+def reduce_over_ranks(ms, units, world, device="cuda"):
+    """Contract of the N > 1 line: time = MAX over ranks (device-timed), units = SUM over ranks (replicas only,
+    DESIGN.md section 9: no data-path collective; this all_reduce of two scalars is the only communication)."""
+    if world <= 1:
+        return float(ms), float(units)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([units], device=device, dtype=torch.float64)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 class ClockSampler:
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -260,14 +274,7 @@ def run_ours(args):
     step_kernel_ms = sum(a.elapsed_time(b) for a, b in evs)
     counters = ctx.counters()
 
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        u = torch.tensor([updates], device="cuda", dtype=torch.float64)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        ms_max, updates_all = float(t.item()), float(u.item())
-    else:
-        ms_max, updates_all = ms, float(updates)
+    ms_max, updates_all = reduce_over_ranks(ms, updates, world)
 
     # ---- end to end through the host-buffer ABI call (pinned host memory, copies inside the timed region)
     e2e = None
@@ -292,10 +299,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
         nup = ctx.updates_total() - u0
-        if world > 1:
-            t = torch.tensor([dt_e], device="cuda", dtype=torch.float64); dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            u = torch.tensor([nup], device="cuda", dtype=torch.float64); dist.all_reduce(u, op=dist.ReduceOp.SUM)
-            dt_e, nup = float(t.item()), float(u.item())
+        dt_e, nup = reduce_over_ranks(dt_e, nup, world)
         e2e = {"value": nup / dt_e, "unit": UNIT, "h2d_bytes_per_step": up // e2e_steps,
                "d2h_bytes_per_step": down // e2e_steps, "steps": e2e_steps,
                "api": "grpic_step_host (C ABI, pinned host buffers, chunked H2D -> fused step -> D2H)"}

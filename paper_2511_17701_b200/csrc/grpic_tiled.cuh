@@ -167,7 +167,10 @@ __device__ __forceinline__ void private_add8(T* sJ, bool on, int node, const T v
 //     add them to eight different addresses with ONE plain read-modify-write.
 //   - The lanes of smaller groups are served by rank inside their group: round r takes the r-th lane of
 //     every group, so the lanes of one round hold pairwise different cells (private_add8).
-constexpr int kBigGroup = 4;
+#ifndef GRPIC_BIG_GROUP
+#define GRPIC_BIG_GROUP 4
+#endif
+constexpr int kBigGroup = GRPIC_BIG_GROUP;
 
 template <typename T>
 __device__ __forceinline__ void warp_deposit(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
