@@ -14,9 +14,10 @@
 //      compare-and-swap loops on sm_100a (LDS + FADD + ATOMS.CAST.SPIN + BRA, retried on every address
 //      collision); with a tile per warp none is needed: lanes depositing into the same cell are
 //      summed across the warp first (transposing butterfly, 9 shuffles instead of 40, for groups of
-//      kBigGroup or more lanes; rank-by-rank rounds for the small groups), and what is left are plain
-//      read-modify-writes whose lanes never share an address.  Particles leaving the window use
-//      global reductions;
+//      kBigGroup or more lanes); stragglers (smaller groups, the part of a path in a neighbour cell) wait
+//      in a per-warp queue and are resolved 32 at a time (butterfly again where they share a cell,
+//      rank-by-rank rounds otherwise); what is left are plain read-modify-writes whose lanes never
+//      share an address.  Particles leaving the window use global reductions;
 //   5. one flush: the private tiles are summed and the non-zero entries go to HBM with red.global.add.
 #pragma once
 #include <cuda.h>
@@ -117,9 +118,10 @@ constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
 constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride;
 static_assert(kJTile % 4 == 0 && kFrontElems % 4 == 0, "128-bit zero fill");
 
+constexpr int kQueueVals = 8 * 64;            // reals per warp queue (8 x kQueue)
 template <typename T>
 constexpr size_t tiled_smem_bytes() {
-  return (size_t)(kFrontElems + kNodeElems) * sizeof(T) + 16;
+  return (size_t)(kFrontElems + kNodeElems + kWarps * kQueueVals) * sizeof(T) + (size_t)kWarps * 64 * sizeof(int) + 16;
 }
 
 // offset inside a shared J tile of value q (0..7, layout of deposit_segments) relative to the cell's node
@@ -172,10 +174,11 @@ __device__ __forceinline__ void private_add8(T* sJ, bool on, int node, const T v
 #endif
 constexpr int kBigGroup = GRPIC_BIG_GROUP;
 
-template <typename T>
-__device__ __forceinline__ void warp_deposit(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
+// kRounds = false: only the big groups are added; the function returns true in the lanes it did not serve.
+template <typename T, bool kRounds>
+__device__ __forceinline__ bool warp_deposit(T* sJ, int lane, int my_off, bool has, int key, const T v[8]) {
   const unsigned act = __ballot_sync(0xffffffffu, has);
-  if (act == 0u) return;
+  if (act == 0u) return false;
   const unsigned peers = __match_any_sync(0xffffffffu, has ? key : ~lane);
   const int cnt = __popc(peers);
   unsigned big = __ballot_sync(0xffffffffu, has && cnt >= kBigGroup);
@@ -206,6 +209,7 @@ __device__ __forceinline__ void warp_deposit(T* sJ, int lane, int my_off, bool h
     __syncwarp();
   }
   const bool small = has && cnt < kBigGroup;
+  if (!kRounds) return small;
   unsigned rem = __ballot_sync(0xffffffffu, small);
   if (rem) {
     const int rank = __popc(peers & ((1u << lane) - 1u));
@@ -215,7 +219,52 @@ __device__ __forceinline__ void warp_deposit(T* sJ, int lane, int my_off, bool h
       rem &= ~__ballot_sync(0xffffffffu, on);
     }
   }
+  return false;
 }
+
+// Deferred stragglers.  Lanes whose cell is shared by fewer than kBigGroup lanes of the current 32 particles
+// (particles that drifted out of their sorted cell, sparse cells) and the part of a path that lies in a
+// neighbour cell are a few entries per iteration; resolving their conflicts every iteration costs as much
+// as the whole push of a particle.  They are appended to a per-warp queue in shared memory (cell + eight
+// values, structure of arrays) and resolved 32 at a time with one warp_deposit — where entries of the
+// same cell collected over several iterations form big groups again.
+constexpr int kQueue = 64;                      // entries per warp: at most 31 left over + 32 appended
+
+template <typename T>
+struct WarpQueue {
+  int* k;      // [kQueue]
+  T* v;        // [8][kQueue]
+  int n;       // warp-uniform
+  __device__ __forceinline__ void append(int lane, bool has, int key, const T val[8]) {
+    const unsigned m = __ballot_sync(0xffffffffu, has);
+    if (m == 0u) return;
+    if (has) {
+      const int pos = n + __popc(m & ((1u << lane) - 1u));
+      k[pos] = key;
+#pragma unroll
+      for (int q = 0; q < 8; ++q) v[q * kQueue + pos] = val[q];
+    }
+    n += __popc(m);
+    __syncwarp();
+  }
+  // resolve 32 entries from the top while at least `keep`+1 .. are queued: drain(31) keeps < 32, drain(0) empties
+  __device__ __forceinline__ void drain(T* sJ, int lane, int my_off, int keep) {
+    while (n > keep) {
+      const int base = n > 32 ? n - 32 : 0;
+      const bool has = base + lane < n;
+      int key = 0;
+      T val[8];
+      if (has) {
+        key = k[base + lane];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) val[q] = v[q * kQueue + base + lane];
+      }
+      warp_deposit<T, true>(sJ, lane, my_off, has, key, val);
+      n = base;
+      __syncwarp();
+    }
+  }
+};
 
 // node-major shared field accessor: four node reads, six bilinear forms
 template <typename T>
@@ -260,7 +309,9 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the kWarps private J tiles
   T* sN = sF + kFrontElems;                           // node-major averaged fields
-  uint64_t* bar = reinterpret_cast<uint64_t*>(sN + kNodeElems);
+  T* sQv = sN + kNodeElems;                           // per-warp straggler queues: values, then cells
+  int* sQk = reinterpret_cast<int*>(sQv + kWarps * kQueueVals);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sQk + kWarps * kQueue);
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   T* sJ = sF + wid * kJTile;                          // this warp's private J tile
@@ -327,6 +378,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   const int my_off = j_offset_of(((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1));
   const uint32_t end = item.begin + item.count;
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
+  WarpQueue<T> Q{sQk + wid * kQueue, sQv + wid * kQueueVals, 0};
   // Each warp owns a CONTIGUOUS slice of the item (sorted by cell): the 32 particles of one iteration
   // then sit in one to three cells, which is what makes the warp-level aggregation cheap.
   const uint32_t per_warp = ((item.count + kTBlock - 1) / kTBlock) * 32u;
@@ -416,9 +468,14 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
       }
       n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
     }
-    warp_deposit(sJ, lane, my_off, dep_a, node_a, seg[0]);
-    warp_deposit(sJ, lane, my_off, dep_b, node_b, seg[1]);
+    // big groups of the start cells now; stragglers and the neighbour-cell parts through the queue
+    const bool left_a = warp_deposit<T, false>(sJ, lane, my_off, dep_a, node_a, seg[0]);
+    Q.append(lane, left_a, node_a, seg[0]);
+    Q.drain(sJ, lane, my_off, 31);
+    Q.append(lane, dep_b, node_b, seg[1]);
+    Q.drain(sJ, lane, my_off, 31);
   }
+  Q.drain(sJ, lane, my_off, 0);
   // counters: one atomic per warp and counter
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
