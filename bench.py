@@ -286,7 +286,7 @@ def run_ours(args):
         hJ = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec)).pin_memory() for k in ("J1", "J2", "J3")}
         up = down = 0
         for p in hsets:                      # warm-up: allocates the library's device chunks
-            ctx.step_host(p, hf, hJ, wl.dt)
+            ctx.step_host(p, hf, hJ, wl.dt, with_prev=False)
         u0 = ctx.updates_total()
         torch.cuda.synchronize()
         if world > 1:
@@ -294,7 +294,7 @@ def run_ours(args):
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             for p in hsets:
-                a, b = ctx.step_host(p, hf, hJ, wl.dt)
+                a, b = ctx.step_host(p, hf, hJ, wl.dt, with_prev=False)
                 up += a; down += b
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
@@ -302,7 +302,7 @@ def run_ours(args):
         dt_e, nup = reduce_over_ranks(dt_e, nup, world)
         e2e = {"value": nup / dt_e, "unit": UNIT, "h2d_bytes_per_step": up // e2e_steps,
                "d2h_bytes_per_step": down // e2e_steps, "steps": e2e_steps,
-               "api": "grpic_step_host (C ABI, pinned host buffers, chunked H2D -> fused step -> D2H)"}
+               "api": "grpic_step_host (C ABI, pinned host buffers, chunked H2D -> fused step -> D2H on three streams; *_prev columns not requested)"}
         del hsets, hf, hJ
 
     if rank != 0:

@@ -149,7 +149,9 @@ int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* cuda_stream);
 /* End-to-end convenience: every pointer in p, fields and J is HOST memory (pinned or pageable).
  * Copies fields and particle columns to library-owned device buffers in chunks, runs the fused step
  * chunk by chunk (copies overlapped with compute on two streams), accumulates J on the device and
- * copies the particle columns and J back; J_host += .  Synchronous.  Bytes moved are reported through
+ * copies the particle columns and J back; J_host += .  The four *_prev columns of p_host may all be NULL:
+ * the fused step keeps the previous position on the device and nothing is copied back for them.
+ * Synchronous.  Bytes moved are reported through
  * h2d_bytes / d2h_bytes (may be NULL).  Errors as grpic_step, plus ENOMEM. */
 int grpic_step_host(grpic_ctx* ctx, grpic_particles* p_host, const grpic_fields* fields_host,
                     grpic_current* J_host, double dt, int64_t* h2d_bytes, int64_t* d2h_bytes);

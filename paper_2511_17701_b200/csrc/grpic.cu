@@ -55,7 +55,7 @@ struct grpic_ctx {
   size_t h_cap;
   void* h_fields;
   size_t h_fields_bytes;
-  cudaStream_t h_streams[2];
+  cudaStream_t h_streams[3];
   bool h_streams_ok;
 };
 
@@ -236,7 +236,7 @@ int grpic_destroy(grpic_ctx* ctx) {
   cudaFree(ctx->d_scratch);
   for (auto q : ctx->h_dev) cudaFree(q);
   cudaFree(ctx->h_fields);
-  if (ctx->h_streams_ok) { cudaStreamDestroy(ctx->h_streams[0]); cudaStreamDestroy(ctx->h_streams[1]); }
+  if (ctx->h_streams_ok) for (auto& q : ctx->h_streams) cudaStreamDestroy(q);
   delete ctx;
   return GRPIC_OK;
 }
@@ -469,8 +469,9 @@ int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* stream) {
 int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh, grpic_current* Jh, double dt,
                     int64_t* h2d_bytes, int64_t* d2h_bytes) {
   if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, ph, true);
+  int rc = check_particles(ctx, ph, false);
   if (rc) return rc;
+  const bool want_prev = ph->i1_prev && ph->i2_prev && ph->dx1_prev && ph->dx2_prev;   // all four or none come back
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
   const SpeciesConst sc = make_species(ph, dt, true);
   if (sc.em && (!fh || !fh->D1 || !fh->D2 || !fh->D3 || !fh->B1 || !fh->B2 || !fh->B3))
@@ -481,8 +482,7 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
   const size_t cells = (size_t)(ctx->grid.n1 + 2 * ctx->grid.nghost) * (ctx->grid.n2 + 2 * ctx->grid.nghost);
   const size_t gbytes = cells * sizeof(real);
   if (!ctx->h_streams_ok) {
-    CK(cudaStreamCreateWithFlags(&ctx->h_streams[0], cudaStreamNonBlocking));
-    CK(cudaStreamCreateWithFlags(&ctx->h_streams[1], cudaStreamNonBlocking));
+    for (auto& q : ctx->h_streams) CK(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
     ctx->h_streams_ok = true;
   }
   if (ctx->h_fields_bytes < 9 * gbytes) {
@@ -499,7 +499,7 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
     for (auto& q : ctx->h_dev) { cudaFree(q); q = nullptr; }
     ctx->h_cap = 0;
     for (auto& q : ctx->h_dev)
-      if (cudaMalloc(&q, 2 * cb) != cudaSuccess) {      // double-buffered: [0, cb) and [cb, 2cb)
+      if (cudaMalloc(&q, 3 * cb) != cudaSuccess) {      // three chunks in flight: upload, compute, download
         cudaGetLastError();
         return fail(ctx, GRPIC_ENOMEM, "device particle chunk allocation failed");
       }
@@ -527,7 +527,7 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
   ctx->last_dt = dt; ctx->have_dt = true;
   const Consts<real> g = make_consts(ctx);
   int buf = 0;
-  for (int64_t lo = 0; lo < ph->n; lo += chunk, buf ^= 1) {
+  for (int64_t lo = 0; lo < ph->n; lo += chunk, buf = (buf + 1) % 3) {
     const int64_t m = (ph->n - lo < chunk) ? ph->n - lo : chunk;
     cudaStream_t st = ctx->h_streams[buf];
     char* base[16];
@@ -555,14 +555,15 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
     DOWN(ph->dx1, P.dx1, rb); DOWN(ph->dx2, P.dx2, rb);
     DOWN(ph->u1, P.u1, rb); DOWN(ph->u2, P.u2, rb); DOWN(ph->u3, P.u3, rb);
     if (P.phi) DOWN(ph->phi, P.phi, rb);
-    DOWN(ph->i1_prev, P.i1p, ib); DOWN(ph->i2_prev, P.i2p, ib);
-    DOWN(ph->dx1_prev, P.dx1p, rb); DOWN(ph->dx2_prev, P.dx2p, rb);
+    if (want_prev) {
+      DOWN(ph->i1_prev, P.i1p, ib); DOWN(ph->i2_prev, P.i2p, ib);
+      DOWN(ph->dx1_prev, P.dx1p, rb); DOWN(ph->dx2_prev, P.dx2p, rb);
+    }
     DOWN(ph->tag, P.tag, (size_t)m);
 #undef UP
 #undef DOWN
   }
-  CK(cudaStreamSynchronize(ctx->h_streams[0]));
-  CK(cudaStreamSynchronize(ctx->h_streams[1]));
+  for (auto& q : ctx->h_streams) CK(cudaStreamSynchronize(q));
   if (sc.do_deposit) {
     std::vector<real> tmp;
     try { tmp.resize(cells); } catch (...) { return fail(ctx, GRPIC_ENOMEM, "host staging allocation failed"); }

@@ -150,8 +150,10 @@ class ParticleSet:
     def to_numpy(self) -> dict:
         return {k: (None if v is None else v.detach().cpu().numpy().copy()) for k, v in self.cols.items()}
 
-    def c_struct(self) -> _Particles:
+    def c_struct(self, with_prev: bool = True) -> _Particles:
         c = self.cols
+        if not with_prev:
+            c = dict(c, i1_prev=None, i2_prev=None, dx1_prev=None, dx2_prev=None)
         ptr = lambda t: None if t is None else t.data_ptr()
         return _Particles(self.n, ptr(c["i1"]), ptr(c["i2"]), ptr(c["dx1"]), ptr(c["dx2"]), ptr(c["u1"]),
                           ptr(c["u2"]), ptr(c["u3"]), ptr(c["phi"]), ptr(c["i1_prev"]), ptr(c["i2_prev"]),
@@ -260,9 +262,10 @@ class Context:
         self._ck(self.lib.grpic_updates_total(self.h, C.byref(v), _stream_ptr(stream)))
         return int(v.value)
 
-    def step_host(self, p: ParticleSet, fields, J, dt):
-        """All tensors are HOST tensors (pinned or not).  Returns (h2d_bytes, d2h_bytes)."""
-        ps = p.c_struct(); fs = _fields_struct(fields); js = _current_struct(J)
+    def step_host(self, p: ParticleSet, fields, J, dt, with_prev: bool = True):
+        """All tensors are HOST tensors (pinned or not).  Returns (h2d_bytes, d2h_bytes).
+        with_prev=False passes NULL for the four *_prev columns (they are then not copied back)."""
+        ps = p.c_struct(with_prev); fs = _fields_struct(fields); js = _current_struct(J)
         up, down = C.c_int64(0), C.c_int64(0)
         self._ck(self.lib.grpic_step_host(self.h, C.byref(ps), C.byref(fs) if fs else None,
                                           C.byref(js) if js else None, float(dt), C.byref(up), C.byref(down)))

@@ -196,6 +196,17 @@ def test_step_host_matches_device_step(G, O, W):
     for k in Jd:
         assert torch.allclose(Jd[k].cpu(), Jh[k], rtol=0, atol=1e-5 * float(Jd[k].abs().max()))
     assert up > 0 and down > 0
+    # the four *_prev columns are optional on the host path: NULL -> nothing comes back for them
+    ph2 = G.ParticleSet.from_host(sp, "f32", device="cpu", pinned=True)
+    for k in ("i1_prev", "i2_prev"):
+        ph2.cols[k].fill_(-7)
+    Jh2 = {k: torch.zeros(ctx.shape, dtype=torch.float32).pin_memory() for k in ("J1", "J2", "J3")}
+    up2, down2 = ctx.step_host(ph2, fhost, Jh2, wl.dt, with_prev=False)
+    c2 = ph2.to_numpy()
+    assert down2 < down and up2 == up
+    assert np.all(c2["i1_prev"] == -7) and np.all(c2["i2_prev"] == -7)
+    for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "phi", "tag"):
+        assert np.array_equal(a[k], c2[k]), k
 
 
 def test_edge_cases(G, O, W):
