@@ -117,6 +117,24 @@ def test_config2_geodesic_sample(G, O, W, prec):
     print("config2", prec, res)
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_massless_particles(G, O, W, prec):
+    """Photons (Eq. 20 with eps = 0; EM push skipped): the config-2 sample pushed as massless
+    particles, 5 steps, against the oracle (whose massless branch is pinned by radial null rays dr/dt = -1);
+    a massless species with a charge still deposits its current (split and fused paths)."""
+    wl = W.config_geodesic(n=1 << 16, dtype=prec)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    sp = wl.species[0]
+    sp.massive = 0
+    sp.charge = 1.0                      # q_over_m stays 0: no EM push, but the particle carries current
+    for mode in ("fused", "split"):
+        ps = G.ParticleSet.from_host(sp, prec)
+        for step in range(5):
+            res, c = _one_step_parity(G, O, ctx, g, ps, None, None, wl.dt, prec, mode)
+        print("massless", prec, mode, res, c)
+
+
 def _shrunk(W, name, shrink):
     return dict(magnetosphere=W.config_magnetosphere, large=W.config_large, two_species=W.config_two_species)[name](shrink=shrink)
 
