@@ -384,7 +384,7 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
       return fail(ctx, GRPIC_ENOMEM, "sort scratch (histogram) allocation failed");
     }
   }
-  // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks; 4. scatter all columns; 5. copy back
+  // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks (inverse permutation); 4. snapshot; 5. gather
   CK(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)sg.n_keys + 1) * 4, st));
   k_sort_hist<<<grid_for(n), kBlock, 0, st>>>(sg, n, p->i1, p->i2, p->tag, ctx->d_keys, ctx->d_hist);
   if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
@@ -411,34 +411,36 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
 
   k_sort_rank<<<grid_for(n), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
 
+  // snapshot of every column in library scratch (plain contiguous copies), then ONE gather back into the
+  // caller's columns in sorted order
   char* s = (char*)ctx->d_scratch;
-  PPtrs<real> in = make_pptrs(p), out;
-  out.n = n;
-  out.dx1 = (real*)s; s += col; out.dx2 = (real*)s; s += col;
-  out.u1 = (real*)s; s += col; out.u2 = (real*)s; s += col; out.u3 = (real*)s; s += col;
-  out.phi = (real*)s; s += col;
-  out.dx1p = (real*)s; s += col; out.dx2p = (real*)s; s += col;
-  out.w = (const real*)s; s += col;
-  out.i1 = (int32_t*)s; s += col4; out.i2 = (int32_t*)s; s += col4;
-  out.i1p = (int32_t*)s; s += col4; out.i2p = (int32_t*)s; s += col4;
-  out.tag = (uint8_t*)s;
-  k_sort_scatter<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
-  CK(cudaGetLastError());
+  PPtrs<real> out = make_pptrs(p), in;
+  in.n = n;
+  in.dx1 = (real*)s; s += col; in.dx2 = (real*)s; s += col;
+  in.u1 = (real*)s; s += col; in.u2 = (real*)s; s += col; in.u3 = (real*)s; s += col;
+  in.phi = p->phi ? (real*)s : nullptr; s += col;
+  in.dx1p = (real*)s; s += col; in.dx2p = (real*)s; s += col;
+  in.w = (const real*)s; s += col;
+  in.i1 = (int32_t*)s; s += col4; in.i2 = (int32_t*)s; s += col4;
+  in.i1p = (int32_t*)s; s += col4; in.i2p = (int32_t*)s; s += col4;
+  in.tag = (uint8_t*)s;
   const size_t rb = (size_t)n * sizeof(real), ib = (size_t)n * 4;
-  CK(cudaMemcpyAsync(p->dx1, out.dx1, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->dx2, out.dx2, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->u1, out.u1, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->u2, out.u2, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->u3, out.u3, rb, cudaMemcpyDeviceToDevice, st));
-  if (p->phi) CK(cudaMemcpyAsync(p->phi, out.phi, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->dx1_prev, out.dx1p, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->dx2_prev, out.dx2p, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync((void*)p->weight, out.w, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->i1, out.i1, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->i2, out.i2, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->i1_prev, out.i1p, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->i2_prev, out.i2p, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(p->tag, out.tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.dx1, p->dx1, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.dx2, p->dx2, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.u1, p->u1, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.u2, p->u2, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.u3, p->u3, rb, cudaMemcpyDeviceToDevice, st));
+  if (p->phi) CK(cudaMemcpyAsync(in.phi, p->phi, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.dx1p, p->dx1_prev, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.dx2p, p->dx2_prev, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync((void*)in.w, p->weight, rb, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.i1, p->i1, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.i2, p->i2, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.i1p, p->i1_prev, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.i2p, p->i2_prev, ib, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(in.tag, p->tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
+  k_sort_gather<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
+  CK(cudaGetLastError());
   return GRPIC_OK;
 }
 

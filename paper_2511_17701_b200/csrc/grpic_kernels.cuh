@@ -217,7 +217,8 @@ __global__ void __launch_bounds__(kBlock) k_sort_hist(const SortGeom s, int64_t 
   if (in && lane == __ffs(peers) - 1) atomicAdd(&hist[key], (uint32_t)__popc(peers));
 }
 
-// destination slot of every particle: offset[key]++ (warp-aggregated)
+// rank of every particle inside its key: offset[key]++ (warp-aggregated); written as the inverse permutation
+// src[slot] = particle, so that the move is a gather (coalesced writes, nearly sequential reads)
 __global__ void __launch_bounds__(kBlock) k_sort_rank(int64_t n, const uint32_t* key_in, uint32_t* cursor,
                                                       uint32_t* dest) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -229,15 +230,15 @@ __global__ void __launch_bounds__(kBlock) k_sort_rank(int64_t n, const uint32_t*
   uint32_t base = 0;
   if (in && lane == leader) base = atomicAdd(&cursor[key], (uint32_t)__popc(peers));
   base = __shfl_sync(0xffffffffu, base, leader);
-  if (in) dest[k] = base + __popc(peers & ((1u << lane) - 1u));
+  if (in) dest[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)k;   // dest[] holds the SOURCE of every slot
 }
 
 template <typename T>
-__global__ void __launch_bounds__(kBlock) k_sort_scatter(const PPtrs<T> in, const PPtrs<T> out,
-                                                         const uint32_t* dest) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= in.n) return;
-  const uint32_t d = dest[k];
+__global__ void __launch_bounds__(kBlock) k_sort_gather(const PPtrs<T> in, const PPtrs<T> out,
+                                                        const uint32_t* src) {
+  const int64_t d = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= in.n) return;
+  const uint32_t k = src[d];
   out.i1[d] = in.i1[k]; out.i2[d] = in.i2[k];
   out.dx1[d] = in.dx1[k]; out.dx2[d] = in.dx2[k];
   out.u1[d] = in.u1[k]; out.u2[d] = in.u2[k]; out.u3[d] = in.u3[k];
