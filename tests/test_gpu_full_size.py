@@ -36,27 +36,31 @@ def _cic_rho(torch, shape, ng, i1, i2, dx1, dx2, qw, mask):
     return rho.view(shape)
 
 
-def test_config4_large_full_size(G, O, W):
-    """Config 4 at full size (2048x1024, 134M particles, FP32): sort + tiled fused step as bench.py runs it.
+@pytest.mark.parametrize("name,prec,tol_cont,tol_mom", [("large", "f32", 5e-6, 1e-6),
+                                                        ("magnetosphere", "f32", 5e-6, 1e-6),
+                                                        ("two_species", "f64", 1e-13, 1e-13)])
+def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
+    """Configs 3, 4, 5 at full size (config 4: 2048x1024, 134M particles, FP32, the bench workload): sort + tiled
+    fused step as bench.py runs it.
     (a) 2^17 sampled particles per species (plus the ragged ends of the sorted order) against the oracle;
     (b) counters add up; (c) discrete continuity of the deposited J with the particles' own (prev -> new)
     positions at every node; (d) first moments of J."""
     import torch
-    wl = W.config_large()
+    wl = dict(large=W.config_large, magnetosphere=W.config_magnetosphere, two_species=W.config_two_species)[name]()
     dom = wl.dom
     g = grid_from_domain(O, dom)
-    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision="f32")
+    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
     names = ("D1", "D2", "D3", "B1", "B2", "B3")
-    fdev = G.grid_tensors(wl.fields, names, "f32")
+    fdev = G.grid_tensors(wl.fields, names, prec)
     fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
     Jtot = {k: torch.zeros(ctx.shape, dtype=torch.float64, device="cuda") for k in ("J1", "J2", "J3")}
-    J = {k: torch.zeros(ctx.shape, dtype=torch.float32, device="cuda") for k in ("J1", "J2", "J3")}
+    J = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
     rng = np.random.default_rng(44)
     rho_diff = torch.zeros(ctx.shape, dtype=torch.float64, device="cuda")
     m1 = m2 = 0.0
     scale = 0.0
     for sp in wl.species:
-        ps = G.ParticleSet.from_host(sp, "f32")
+        ps = G.ParticleSet.from_host(sp, prec)
         n = ps.n
         ctx.sort(ps)
         ctx.step(ps, fdev, J, wl.dt)            # one step to leave the freshly sorted state (drifted particles)
@@ -75,8 +79,8 @@ def test_config4_large_full_size(G, O, W):
         op = oracle_from_cols(O, before, ps.q_over_m, ps.charge, ps.massive)
         diag = {}
         O.push(g, op, fhost, wl.dt, diag=diag)
-        res = compare_particles(op, after, "f32", before["tag"], g.n1, g.n2, diag=diag)
-        print("config4 full", sp.name, res, c)
+        res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag)
+        print(name, "full", sp.name, res, c)
         # (b) counters
         alive_after = int(ps.cols["tag"].sum())
         assert c["alive"] == alive_after and c["overstep"] == 0
@@ -103,14 +107,14 @@ def test_config4_large_full_size(G, O, W):
     resid = rho_diff / wl.dt + div
     # scale: the largest one-species |J| entry; FP32 sums of a few hundred contributions per entry -> ~1e-6 relative
     r = float(resid[1:, 1:].abs().max()) / scale
-    print("config4 full: continuity residual / max|J| =", r)
-    assert r < 5e-6
+    print(name, "full: continuity residual / max|J| =", r)
+    assert r < tol_cont
     # first moments: sum over the grid of J^i = sum_p q w dx^i/dt   (species of opposite charge cancel in the
     # total, so compare against the per-species magnitude scale)
     e1 = abs(float(J1.sum()) - m1) / scale_sp
     e2 = abs(float(J2.sum()) - m2) / scale_sp
-    print("config4 full: first-moment errors", e1, e2)
-    assert e1 < 1e-6 and e2 < 1e-6
+    print(name, "full: first-moment errors", e1, e2)
+    assert e1 < tol_mom and e2 < tol_mom
 
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])
