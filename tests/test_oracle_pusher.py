@@ -324,3 +324,136 @@ def test_previous_position_saved_and_renormalised(O):
     assert np.all((p.dx1 >= 0) & (p.dx1 < 1) & (p.dx2 >= 0) & (p.dx2 < 1))
     moved = np.abs((p.i1 + p.dx1) - (q.i1 + q.dx1))
     assert moved.max() > 0.05
+
+
+# --------------------------------------------------------------------------------------------
+# Brute-force single-particle traces (north_star): Hamilton's equations of the 3+1 split,
+#   H = -u_0 = alpha*sqrt(eps + h^ij u_i u_j) - beta^i u_i  (P:215 footnote 8 with Eq. 20),
+#   dx^i/dt = dH/du_i,  du_i/dt = -dH/dx^i,
+# in PHYSICAL Kerr-Schild coordinates (r, theta), with the textbook contravariant 3-metric typed out
+# here and the derivatives of H taken numerically (central differences): nothing of App. A's
+# derivative list, of the code basis or of the midpoint scheme is shared with the oracle.
+# Integrated by scipy's DOP853 to 1e-12; the oracle's trajectory must converge to it at second order.
+# A wrong sign or a dropped term in Eq. 26-29 or in the A.2/A.3 derivatives fails this test.
+# --------------------------------------------------------------------------------------------
+def _H_phys(a, eps, r, th, ur, uth, uph):
+    S = r * r + a * a * np.cos(th) ** 2
+    D = r * r - 2 * r + a * a
+    A = (r * r + a * a) ** 2 - a * a * D * np.sin(th) ** 2
+    z = 2 * r / S
+    alpha, beta_r = 1 / np.sqrt(1 + z), z / (1 + z)
+    g2 = eps + A / (S * (S + 2 * r)) * ur * ur + uth * uth / S + uph * uph / (S * np.sin(th) ** 2) + 2 * a / S * ur * uph
+    return alpha * np.sqrt(g2) - beta_r * ur
+
+
+def _brute_force_trace(a, eps, y0, times):
+    """state (r, theta, phi, u_r, u_theta, u_phi) at each of `times` (any sign), from y0 at t = 0"""
+    from scipy.integrate import solve_ivp
+
+    def rhs(t, y):
+        r, th, ph, ur, uth, uph = y
+        h = 1e-6
+        d = lambda k: (_H_phys(a, eps, *(np.array([r, th, ur, uth, uph]) + h * np.eye(5)[k])) -
+                       _H_phys(a, eps, *(np.array([r, th, ur, uth, uph]) - h * np.eye(5)[k]))) / (2 * h)
+        return [d(2), d(3), d(4), -d(0), -d(1), 0.0]
+
+    back = [t for t in times if t < 0]
+    fwd = sorted(t for t in times if t > 0)
+    out = {}
+    for t in back:
+        out[t] = solve_ivp(rhs, (0.0, t), y0, method="DOP853", rtol=1e-12, atol=1e-13).y[:, -1]
+    if fwd:
+        sol = solve_ivp(rhs, (0.0, fwd[-1]), y0, method="DOP853", rtol=1e-12, atol=1e-13, t_eval=fwd)
+        for k, t in enumerate(fwd):
+            out[t] = sol.y[:, k]
+    return [out[t] for t in times]
+
+
+@pytest.mark.parametrize("a,eps,r0,th0,ur,uth,uph", [(0.9, 1.0, 6.0, 1.2, -0.1, 0.8, 2.5),      # inclined bound-ish orbit
+                                                     (0.995, 1.0, 3.0, np.pi / 2 - 0.3, 0.05, -0.5, 1.9),  # near the hole
+                                                     (0.7, 0.0, 8.0, 0.9, -0.6, 1.5, -2.0)])   # photon, retrograde
+def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph):
+    T = 1.0
+    y0 = [r0, th0, 0.0, ur, uth, uph]
+    errs = []
+    for dt in (0.02, 0.01, 0.005):
+        # leapfrog (Sec. 3.1, P:213-262): positions live at t_n, velocities at t_(n-1/2).  The oracle starts from
+        # x(0) and u(-dt/2) of the brute-force trajectory and must end at x(T), u(T - dt/2) of the same trajectory.
+        y_m, y_u, y_x = _brute_force_trace(a, eps, y0, [-0.5 * dt, T - 0.5 * dt, T])
+        g = O.Grid(256, 128, a, 0.9 * (1 + np.sqrt(1 - a * a)), 30.0, n_iter=25)
+        # u_1 = u_r dr/dx1 is the momentum conjugate to x1: its scale factor dxi*r is taken where u lives (t = -dt/2)
+        p = one_particle(O, g, r0, th0, y_m[3] * y_m[0] / r0, y_m[4], y_m[5], massive=int(eps))
+        for _ in range(int(round(T / dt))):
+            O.push(g, p, None, dt)
+        r, th = _phys(O, g, p)
+        dxi, deta = np.log(g.r_max / g.r_min) / g.n1, np.pi / g.n2
+        # covariant u_r at (T - dt/2) in the physical basis: the code-basis scale factor is taken where u lives
+        r_u = y_u[0]
+        got = np.array([r, th, p.phi[0], p.u1[0] / (dxi * r_u), p.u2[0] / deta, p.u3[0]])
+        ref = np.array([y_x[0], y_x[1], y_x[2], y_u[3], y_u[4], y_u[5]])
+        errs.append(np.max(np.abs(got - ref) / np.maximum(1.0, np.abs(ref))))
+    assert errs[2] < 1e-5, errs                                           # converged to the brute-force trace
+    assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs   # at second order
+
+
+def _A_wald_phys(a, B0, r, th):
+    """Eq. 60: A_mu = (B0/2)(g_{mu phi} + 2a g_{mu t}) with the covariant Kerr-Schild 4-metric (A1)."""
+    S = r * r + a * a * np.cos(th) ** 2
+    D = r * r - 2 * r + a * a
+    A = (r * r + a * a) ** 2 - a * a * D * np.sin(th) ** 2
+    z, s2 = 2 * r / S, np.sin(th) ** 2
+    g00, g01, g03 = -(1 - z), z, -a * z * s2
+    g13, g33 = -a * (1 + z) * s2, A * s2 / S
+    return 0.5 * B0 * (g03 + 2 * a * g00), 0.5 * B0 * (g13 + 2 * a * g01), 0.5 * B0 * (g33 + 2 * a * g03)
+
+
+def _brute_force_charged(a, B0, qm, y0, times):
+    """Canonical Hamiltonian of a charge in the stationary Wald field, t as the parameter:
+    H = alpha*gamma(u) - beta^r u_r - (q/m) A_0,  u_i = pi_i - (q/m) A_i;  y = (r, theta, pi_r, pi_theta, pi_phi)."""
+    from scipy.integrate import solve_ivp
+
+    def H(r, th, pr, pth, pph):
+        A0, Ar, Aph = _A_wald_phys(a, B0, r, th)
+        return _H_phys(a, 1.0, r, th, pr - qm * Ar, pth, pph - qm * Aph) - qm * A0
+
+    def rhs(t, y):
+        h = 1e-6
+        d = lambda k: (H(*(y + h * np.eye(5)[k])) - H(*(y - h * np.eye(5)[k]))) / (2 * h)
+        return [d(2), d(3), -d(0), -d(1), 0.0]
+
+    out = []
+    for t in times:
+        out.append(solve_ivp(rhs, (0.0, t), y0, method="DOP853", rtol=1e-12, atol=1e-13).y[:, -1])
+    return out
+
+
+def test_brute_force_charged_trace_in_wald_field(O, W):
+    """GR-EM-3D row of Table 1 (a = 0.9, Wald field): the oracle's EM + geodesic push with the
+    analytic D, B at the particle against the brute-force canonical trajectory.  Pins the Boris coefficient
+    (q/m) alpha dt/4 of R-S5, the tetrad projections and the order of the two half pushes: second-order convergence
+    to an independent solution, not only conservation of two invariants."""
+    row = table1()["GR-EM-3D"]
+    a, B0, qm, T = row["a"], 2 * row["Bn"], 1.0, 0.5
+    r0, th0 = row["r"], row["theta"]
+    A0, Ar, Aph = _A_wald_phys(a, B0, r0, th0)
+    y0 = np.array([r0, th0, row["u1"] + qm * Ar, 0.0, row["u3"] + qm * Aph])
+    errs = []
+    for dt in (0.004, 0.002, 0.001):
+        y_m, y_u, y_x = _brute_force_charged(a, B0, qm, y0, [-0.5 * dt, T - 0.5 * dt, T])
+        g = _grid(O, row)
+        dom = W.Domain(g.n1, g.n2, g.a, g.r_min, g.r_max, g.ng)
+        pot = lambda d, x, y: W.wald_potential(d, x, y, B0)
+        # kinetic u at t = -dt/2 from the canonical momenta of the brute-force trajectory
+        _, Ar_m, Aph_m = _A_wald_phys(a, B0, y_m[0], y_m[1])
+        p = one_particle(O, g, r0, th0, (y_m[2] - qm * Ar_m) * y_m[0] / r0, y_m[3], y_m[4] - qm * Aph_m, q_over_m=qm)
+        for _ in range(int(round(T / dt))):
+            f = W.em_at(dom, pot, *pos(p))
+            O.push_given_fields(g, p, [f["D1"][0], f["D2"][0], f["D3"][0]], [f["B1"][0], f["B2"][0], f["B3"][0]], dt)
+        r, th = _phys(O, g, p)
+        dxi, deta = np.log(g.r_max / g.r_min) / g.n1, np.pi / g.n2
+        _, Ar_u, Aph_u = _A_wald_phys(a, B0, y_u[0], y_u[1])
+        got = np.array([r, th, p.u1[0] / (dxi * y_u[0]), p.u2[0] / deta, p.u3[0]])
+        ref = np.array([y_x[0], y_x[1], y_u[2] - qm * Ar_u, y_u[3], y_u[4] - qm * Aph_u])
+        errs.append(np.max(np.abs(got - ref) / np.maximum(1.0, np.abs(ref))))
+    assert errs[2] < 1e-5, errs
+    assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
