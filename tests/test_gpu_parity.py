@@ -160,6 +160,35 @@ def test_configs_3_4_5_shrunk(G, O, W, name, shrink, prec, mode):
     print(name, prec, mode, worst)
 
 
+@pytest.mark.parametrize("n1,n2,ng,n_iter,tma,prec", [(90, 43, 1, 10, 1, "f32"),    # ragged tiles, ld*4 = 180 B: TMA refused -> plain staging
+                                                      (90, 44, 2, 10, 1, "f32"),    # ragged tiles, TMA path
+                                                      (90, 44, 2, 3, 0, "f64"),     # TMA switched off, few iterations
+                                                      (50, 30, 3, 1, 1, "f64"),     # n_iter = 1 (explicit Euler), wide ghosts
+                                                      (16, 16, 2, 10, 1, "f32")])   # one tile
+def test_ragged_grids_ghost_widths_iteration_counts(G, O, W, n1, n2, ng, n_iter, tma, prec):
+    """Grids that are not multiples of the 16-cell tile, 1-3 ghost layers, n_iter = 1, 3, 10, TMA on / off /
+    refused (row pitch not a multiple of 16 bytes): split, fused and tiled paths against the oracle, 3 steps."""
+    a = 0.8
+    dom = W.Domain(n1, n2, a, 0.9 * W.horizon_radius(a), 25.0, ng)
+    rng = np.random.Generator(np.random.Philox(n1 * 1000 + n2))
+    fields = W.add_random_dB(dom, W.wald_fields(dom, 1.0), 0.1, rng)
+    species = W._pairs(dom, W.counts_uniform(dom, 6), 0.5, rng)
+    dt = W.cfl_dt(dom)
+    g = grid_from_domain(O, dom, n_iter=n_iter)
+    ctx = _ctx(G, dom, prec, n_iter=n_iter)
+    ctx.set_int("tma", tma)
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    fdev = G.grid_tensors(fields, names, prec)
+    fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
+    for mode in ("split", "fused", "tiled"):
+        sets = [G.ParticleSet.from_host(sp, prec) for sp in species]
+        for step in range(3):
+            for ps in sets:
+                res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, "fused" if mode == "tiled" else mode,
+                                          sort_first=(mode == "tiled" and step == 0))
+    print("ragged", n1, n2, ng, n_iter, tma, prec, res, c)
+
+
 def test_sort_is_a_permutation_into_key_order(G, O, W):
     import torch
     wl = W.config_large(shrink=16)
