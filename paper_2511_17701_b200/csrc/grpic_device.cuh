@@ -126,6 +126,25 @@ __device__ __forceinline__ void sincos_small(double d, double& sd, double& cd) {
   q = fma(q, d2, -0.5);
   cd = fma(q, d2, 1.0);
 }
+// sin and cos of theta' in [0, pi/2 + a cell]: theta' is folded at pi/4 — the complement pi/2 - theta' is formed
+// from the integer cell count, so it is exact to one rounding — and the classic single-precision minimax
+// polynomials of the quadrant reduction are evaluated on [0, pi/4 + a cell] (< 1 ulp there).  No range
+// reduction, no slow path, no local memory (sincosf carries a Payne-Hanek branch).
+__device__ __forceinline__ void sincos_first_quadrant(float cells, float comp_cells, float half_cells, float deta,
+                                                      float& s, float& c) {
+  const bool hi = cells > 0.5f * half_cells;                 // theta' > pi/4
+  const float z = (hi ? comp_cells : cells) * deta;
+  const float z2 = z * z;
+  float ps = fmaf(z2, -1.9515295891e-4f, 8.3321608736e-3f);
+  ps = fmaf(ps, z2, -1.6666654611e-1f);
+  const float sz = fmaf(ps * z2, z, z);
+  float pc = fmaf(z2, 2.443315711809948e-5f, -1.388731625493765e-3f);
+  pc = fmaf(pc, z2, 4.166664568298827e-2f);
+  const float cz = fmaf(pc * z2, z2, fmaf(z2, -0.5f, 1.0f));
+  s = hi ? cz : sz;
+  c = hi ? sz : cz;
+}
+
 template <typename T> struct SmallLimits;
 template <> struct SmallLimits<float> { static constexpr float e = 0.04f, d = 0.045f; };
 template <> struct SmallLimits<double> { static constexpr double e = 0.04, d = 0.045; };
@@ -190,17 +209,18 @@ struct Coord<double> {
       sin_min = in_reg(g.sin_min); sin_max = in_reg(g.sin_max);
     }
   };
-  __device__ __forceinline__ bool at_fast(const Fast& f, double del1, double del2, double& r, double& sth) const {
+  __device__ __forceinline__ void at_fast(const Fast& f, double del1, double del2, double& r, double& sth,
+                                          double& big) const {
     const double e = del1 * f.hdxi;
     const double th = (x2 + 0.5 * del2) * f.deta;
     const double d = th - th0;
+    big = fmax(big, fmax(fabs(e), fabs(d)));
     r = r0 * exp_small(e);
     double sd, cd;
     sincos_small(d, sd, cd);
     sth = fma(s0, cd, c0 * sd);
     if (th < f.th_min) sth = f.sin_min;
     if (th > f.th_max) sth = f.sin_max;
-    return fabs(e) < SmallLimits<double>::e && fabs(d) < SmallLimits<double>::d;
   }
 };
 
@@ -210,14 +230,14 @@ struct Coord<float> {
   __device__ __forceinline__ void init(const Consts<float>& g, int i1, float dx1, int i2, float dx2) {
     const float xi = fmaf(dx1, g.dxi, fmaf((float)i1, g.dxi, g.log_rmin));
     r0 = expf(xi);
-    if (2 * i2 >= g.n2) {
-      thp = ((float)(g.n2 - i2) - dx2) * g.deta;
-      sgn = -1.f;
-    } else {
-      thp = ((float)i2 + dx2) * g.deta;
-      sgn = 1.f;
-    }
-    sincosf(thp, &s0, &c0);
+    const bool upper = 2 * i2 >= g.n2;
+    const float fc = (float)(upper ? g.n2 - i2 : i2);          // whole cells from the nearer axis
+    const float sdx = upper ? -dx2 : dx2;
+    sgn = upper ? -1.f : 1.f;
+    const float cells = fc + sdx;
+    const float half = 0.5f * (float)g.n2;                     // cells in a quadrant
+    thp = cells * g.deta;
+    sincos_first_quadrant(cells, (half - fc) - sdx, half, g.deta, s0, c0);
   }
   __device__ __forceinline__ void at0(const Consts<float>& g, float& r, float& sth, float& cth) const {
     float s = s0, c = c0;
@@ -257,16 +277,18 @@ struct Coord<float> {
       th_min = in_reg(g.th_min); sin_min = in_reg(g.sin_min);
     }
   };
-  __device__ __forceinline__ bool at_fast(const Fast& f, float del1, float del2, float& r, float& sth) const {
+  // `big` accumulates max(|e|, |d|) over the loop: one FMNMX3-style update instead of two compares and selects;
+  // the caller tests it once against the smaller of the two SmallLimits (conservative).
+  __device__ __forceinline__ void at_fast(const Fast& f, float del1, float del2, float& r, float& sth, float& big) const {
     const float e = del1 * f.hdxi;
     const float d = del2 * f.hdeta;
+    big = fmaxf(big, fmaxf(fabsf(e), fabsf(d)));
     r = r0 * exp_small(e);
     float sd, cd;
     sincos_small(d, sd, cd);
     float s = fmaf(s0, cd, c0 * sd);
     if (thp + d < f.th_min) s = f.sin_min;
     sth = s;
-    return fabsf(e) < SmallLimits<float>::e && fabsf(d) < SmallLimits<float>::d;
   }
 };
 
@@ -580,10 +602,10 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
     XF.init(g, X);
     const int n_iter = in_reg(g.n_iter);
     const bool ee = g.early_exit != 0;
-    bool ok = true;
+    T big = T(0);
     for (int it = 0; it < n_iter; ++it) {
       T r, sth, n1, n2;
-      ok &= X.at_fast(XF, del1, del2, r, sth);
+      X.at_fast(XF, del1, del2, r, sth, big);
       E.eval(g, U, r, sth, n1, n2);
       // bit-identical iterate => every later iterate is the same: stopping here IS n_iter iterations
       fixed = (n1 == del1) & (n2 == del2);
@@ -593,12 +615,12 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
     }
     // step 11, Eq. 30 at x_m = (x^(n) + x^(n+1))/2.  If the last iterate repeated, the midpoint
     // of the last evaluation is x_m itself and its coefficients are reused; otherwise evaluate there.
-    if (ok && !fixed) {
+    if (!fixed) {
       T r, sth, n1, n2;
-      ok &= X.at_fast(XF, del1, del2, r, sth);
+      X.at_fast(XF, del1, del2, r, sth, big);
       E.eval(g, U, r, sth, n1, n2);
     }
-    if (!ok) {
+    if (!(big < SmallLimits<T>::e)) {                    // e-limit 0.04 < d-limit 0.045; NaN-safe
       // a displacement left SmallLimits (many cells in one step): redo the loop with the library functions
       del1 = T(0); del2 = T(0);
       for (int it = 0; it < g.n_iter; ++it) {
