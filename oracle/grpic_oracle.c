@@ -48,30 +48,42 @@ typedef struct {
   double a;              /* spin, r_g = M = 1                          */
   double r_min, r_max;   /* radial extent; log-r map A.3 with r0=0,h0=0 */
   double small_angle;    /* SMALL_ANGLE_GR                            */
+  double r0;             /* radial offset of A.3: xi = log(r - r0)    */
+  double h0;             /* polar stretch of A.3; 0 = uniform     */
 } orc_grid;
 
 typedef struct {
   double r, th, sth, cth;
   double Sigma, Delta, A, z;
-  double s1, s2;                     /* dr/dx1 = dxi*r,  dtheta/dx2 = deta    */
+  double s1, s2;                     /* dr/dx1 = dxi*(r-r0), dtheta/dx2 = deta*dtheta/deta */
   double alpha, beta1;               /* lapse, shift beta^1 (code basis)      */
   double hu11, hu22, hu33, hu13;     /* h^{ij}                                */
   double hd11, hd22, hd33, hd13;     /* h_{ij}                                */
   double sqrt_h;
+  double dls2;                       /* d ln(s2)/dx2: non-zero only with the polar stretch h0 (A.3) */
 } orc_metric_t;
 
 typedef struct {                     /* [0] = d/dx1, [1] = d/dx2              */
   double hu11[2], hu22[2], hu33[2], hu13[2], alpha[2], beta1[2];
 } orc_dmetric_t;
 
-static double orc_dxi(const orc_grid* g) { return log(g->r_max / g->r_min) / g->n1; }
+static double orc_dxi(const orc_grid* g) { return log((g->r_max - g->r0) / (g->r_min - g->r0)) / g->n1; }
 static double orc_deta(const orc_grid* g) { return M_PI / g->n2; }
 
-/* P:820-825 with r0 = 0, h0 = 0: xi = ln r, uniform in x1; theta uniform in x2.
+/* P:820-823 (A.3): xi = log(r - r0) uniform in x1;  eta = x2*deta uniform in x2 and
+ *   theta = eta + 2 h0 eta (pi - 2 eta)(pi - eta)/pi^2,
+ *   dtheta/deta = 1 + 2 h0 + 12 h0 (eta/pi)(eta/pi - 1)   (P:823 prints "12h" for 12 h0).
+ * All five BASELINE configs have r0 = 0, h0 = 0.
  * theta used in any metric evaluation is kept away from the axis. */
+static double orc_theta_of_eta(const orc_grid* g, double eta) {
+  return eta + 2.0 * g->h0 * eta * (M_PI - 2.0 * eta) * (M_PI - eta) / (M_PI * M_PI);
+}
+static double orc_dtheta_deta(const orc_grid* g, double eta) {
+  return 1.0 + 2.0 * g->h0 + 12.0 * g->h0 * (eta / M_PI) * (eta / M_PI - 1.0);
+}
 static void orc_coords(const orc_grid* g, double x1, double x2, double* r, double* th) {
-  *r = exp(log(g->r_min) + x1 * orc_dxi(g));
-  double t = x2 * orc_deta(g);
+  *r = g->r0 + exp(log(g->r_min - g->r0) + x1 * orc_dxi(g));
+  double t = orc_theta_of_eta(g, x2 * orc_deta(g));
   if (t < g->small_angle) t = g->small_angle;
   if (t > M_PI - g->small_angle) t = M_PI - g->small_angle;
   *th = t;
@@ -90,8 +102,12 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
   m->Delta = r * r - 2.0 * r + a * a;
   m->A = (r * r + a * a) * (r * r + a * a) - a * a * m->Delta * s2th;
   m->z = 2.0 * r / m->Sigma;
-  m->s1 = orc_dxi(g) * r;
-  m->s2 = orc_deta(g);
+  m->s1 = orc_dxi(g) * (r - g->r0);
+  m->s2 = orc_deta(g) * orc_dtheta_deta(g, x2 * orc_deta(g));
+  {
+    const double eta = x2 * orc_deta(g);
+    m->dls2 = orc_deta(g) * (12.0 * g->h0 / M_PI) * (2.0 * eta / M_PI - 1.0) / orc_dtheta_deta(g, eta);
+  }
   m->alpha = 1.0 / sqrt(1.0 + m->z);
   m->beta1 = m->z / (1.0 + m->z) / m->s1;
   m->hu11 = m->A / (m->Sigma * (m->Sigma + 2.0 * r)) / (m->s1 * m->s1);
@@ -106,7 +122,8 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
 }
 
 /* P:816 (A.2) with dr -> s1, dtheta -> s2, plus the A.3 terms that come from
- * s1 = dxi*e^xi depending on x1 (legible entries of P:842).  Corrections to the
+ * s1 = dxi*e^xi depending on x1 (legible entries of P:842) and, with the polar
+ * stretch, from s2 depending on x2 (h^22 ~ 1/s2^2: the entry P:842 omits).  Corrections to the
  * printed text (DESIGN.md R-S2): d_theta Sigma from P:774; sign of d_xi alpha
  * as in A.2. */
 void orc_dmetric(const orc_grid* g, const orc_metric_t* m, orc_dmetric_t* d) {
@@ -124,7 +141,7 @@ void orc_dmetric(const orc_grid* g, const orc_metric_t* m, orc_dmetric_t* d) {
                - 2.0 * dxi * m->hu11;
   d->hu11[1] = (S * (S + 2.0 * r) * d2A - 2.0 * A * d2S * (r + S)) / den / (s1 * s1);
   d->hu22[0] = -d1S / (S * S) / (s2 * s2);
-  d->hu22[1] = -d2S / (S * S) / (s2 * s2);
+  d->hu22[1] = -d2S / (S * S) / (s2 * s2) - 2.0 * m->dls2 * m->hu22;   /* A.3: s2 depends on x2 */
   d->hu33[0] = -d1S / (S * S * s2th);
   d->hu33[1] = -2.0 * cth * s2 / (S * S * sth * s2th) * (S - a * a * s2th);
   d->hu13[0] = -a / s1 * d1S / (S * S) - dxi * m->hu13;

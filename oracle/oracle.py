@@ -31,11 +31,12 @@ def build(force: bool = False) -> str:
 
 class _Grid(C.Structure):
     _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("ng", C.c_int32), ("n_iter", C.c_int32),
-                ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double)]
+                ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double),
+                ("r0", C.c_double), ("h0", C.c_double)]
 
 
 _METRIC_NAMES = ["r", "th", "sth", "cth", "Sigma", "Delta", "A", "z", "s1", "s2", "alpha", "beta1",
-                 "hu11", "hu22", "hu33", "hu13", "hd11", "hd22", "hd33", "hd13", "sqrt_h"]
+                 "hu11", "hu22", "hu33", "hu13", "hd11", "hd22", "hd33", "hd13", "sqrt_h", "dls2"]
 _DMETRIC_NAMES = ["hu11", "hu22", "hu33", "hu13", "alpha", "beta1"]
 
 _dp = C.POINTER(C.c_double)
@@ -80,9 +81,12 @@ class Grid:
     ng: int = 2
     n_iter: int = 10
     small_angle: float = 1e-5
+    r0: float = 0.0          # A.3 radial offset, xi = log(r - r0)
+    h0: float = 0.0          # A.3 polar stretch
 
     def c(self) -> _Grid:
-        return _Grid(self.n1, self.n2, self.ng, self.n_iter, self.a, self.r_min, self.r_max, self.small_angle)
+        return _Grid(self.n1, self.n2, self.ng, self.n_iter, self.a, self.r_min, self.r_max, self.small_angle,
+                     self.r0, self.h0)
 
     @property
     def shape(self):

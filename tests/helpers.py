@@ -19,15 +19,32 @@ def table1():
     return rows
 
 
+def code_position(O, g, r, theta):
+    """(x1, x2) of physical (r, theta) under the A.3 map of grid g (r0, h0 may be non-zero): the radial map is
+    inverted in closed form, the polar one by bisection on the oracle's own theta(x2)."""
+    r0, h0 = getattr(g, "r0", 0.0), getattr(g, "h0", 0.0)
+    dxi = np.log((g.r_max - r0) / (g.r_min - r0)) / g.n1
+    x1 = np.log((r - r0) / (g.r_min - r0)) / dxi
+    if h0 == 0.0:
+        return x1, theta / (np.pi / g.n2)
+    lo, hi = 0.0, float(g.n2)
+    for _ in range(80):
+        mid = 0.5 * (lo + hi)
+        if O.metric(g, x1, mid, derivs=False)["th"][0] < theta:
+            lo = mid
+        else:
+            hi = mid
+    return x1, 0.5 * (lo + hi)
+
+
 def one_particle(O, g, r, theta, u1_phys, u2_phys, u3, q_over_m=0.0, massive=1, phi=0.0):
-    """Particle at physical (r, theta) with covariant components in the physical basis."""
-    dxi = np.log(g.r_max / g.r_min) / g.n1
-    deta = np.pi / g.n2
-    x1 = np.log(r / g.r_min) / dxi
-    x2 = theta / deta
+    """Particle at physical (r, theta) with covariant components in the physical basis:
+    u_1 = u_r dr/dx1, u_2 = u_theta dtheta/dx2 (scale factors s1, s2 of the map at that point)."""
+    x1, x2 = code_position(O, g, r, theta)
+    m = O.metric(g, x1, x2, derivs=False)
     i1, i2 = int(np.floor(x1)), int(np.floor(x2))
     return O.Particles(i1=[i1], i2=[i2], dx1=[x1 - i1], dx2=[x2 - i2],
-                       u1=[u1_phys * dxi * r], u2=[u2_phys * deta], u3=[u3],
+                       u1=[u1_phys * m["s1"][0]], u2=[u2_phys * m["s2"][0]], u3=[u3],
                        weight=[1.0], tag=[1], phi=[phi], q_over_m=q_over_m, charge=q_over_m, massive=massive)
 
 

@@ -6,9 +6,13 @@ import pytest
 PTS = [(3.2, 7.9), (60.5, 31.7), (100.1, 3.3), (10.0, 60.2), (120.9, 32.0)]
 
 
-@pytest.fixture(scope="module")
-def g(O):
-    return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0)
+@pytest.fixture(scope="module", params=["log_uniform", "offset_stretched"])
+def g(O, request):
+    """The map of the five configs (A.3 with r0 = 0, h0 = 0) and the full A.3 map: radial offset
+    r0 = 0.6 and polar stretch h0 = 0.35; every pin below that does not name the map holds for both."""
+    if request.param == "log_uniform":
+        return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0)
+    return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0, r0=0.6, h0=0.35)
 
 
 def _mat(m, k, up):
@@ -52,8 +56,28 @@ def test_schwarzschild_limit(O):
 
 def test_coordinate_map(O, g):
     m = O.metric(g, np.array([0.0, 128.0, 64.0]), np.array([32.0, 32.0, 16.0]))
-    assert np.allclose(m["r"], [g.r_min, g.r_max, np.sqrt(g.r_min * g.r_max)], rtol=1e-14)
-    assert np.allclose(m["th"], [np.pi / 2, np.pi / 2, np.pi / 4], rtol=1e-14)
+    # xi = log(r - r0) is uniform in x1: the middle of the grid is the geometric mean of (r - r0)
+    assert np.allclose(m["r"], [g.r_min, g.r_max, g.r0 + np.sqrt((g.r_min - g.r0) * (g.r_max - g.r0))], rtol=1e-14)
+    # theta(eta) of P:821 at eta = pi/2 and pi/4: pi/2 (fixed point of the stretch) and pi/4 + 2 h0 (pi/4)(pi/2)(3pi/4)/pi^2
+    assert np.allclose(m["th"], [np.pi / 2, np.pi / 2, np.pi / 4 * (1 + 0.75 * g.h0)], rtol=1e-14)
+
+
+def test_scale_factors_are_the_map_derivatives(O, g):
+    """s1 = dr/dx1 and s2 = dtheta/dx2 (what "dr", "dtheta" of the code basis mean):
+    finite differences of the map itself; and the stretch keeps theta symmetric about the equator,
+    monotonic, with theta(0) = 0, theta(pi) = pi."""
+    x1, x2 = np.array(PTS).T
+    h = 1e-3
+    f = lambda a, b, k: O.metric(g, a, b, derivs=False)[k]
+    s1_fd = (-f(x1 + 2 * h, x2, "r") + 8 * f(x1 + h, x2, "r") - 8 * f(x1 - h, x2, "r") + f(x1 - 2 * h, x2, "r")) / (12 * h)
+    s2_fd = (-f(x1, x2 + 2 * h, "th") + 8 * f(x1, x2 + h, "th") - 8 * f(x1, x2 - h, "th") + f(x1, x2 - 2 * h, "th")) / (12 * h)
+    m = O.metric(g, x1, x2, derivs=False)
+    assert np.allclose(m["s1"], s1_fd, rtol=1e-10) and np.allclose(m["s2"], s2_fd, rtol=1e-10)
+    gg = O.Grid(g.n1, g.n2, g.a, g.r_min, g.r_max, small_angle=0.0, r0=g.r0, h0=g.h0)
+    x = np.linspace(0.0, g.n2, 257)
+    th = O.metric(gg, np.full_like(x, 5.0), x, derivs=False)["th"]
+    assert abs(th[0]) < 1e-15 and abs(th[-1] - np.pi) < 1e-14
+    assert np.all(np.diff(th) > 0) and np.allclose(th + th[::-1], np.pi, atol=1e-14)
 
 
 def test_small_angle_clamp(O, g):

@@ -3,7 +3,7 @@ Kerr closed forms, conservation laws and textbook limits."""
 import numpy as np
 import pytest
 
-from helpers import energy_u0, eq59_energy, one_particle, pos, table1
+from helpers import code_position, energy_u0, eq59_energy, one_particle, pos, table1
 
 
 def _grid(O, row, n_iter=10):
@@ -372,7 +372,8 @@ def _brute_force_trace(a, eps, y0, times):
 @pytest.mark.parametrize("a,eps,r0,th0,ur,uth,uph", [(0.9, 1.0, 6.0, 1.2, -0.1, 0.8, 2.5),      # inclined bound-ish orbit
                                                      (0.995, 1.0, 3.0, np.pi / 2 - 0.3, 0.05, -0.5, 1.9),  # near the hole
                                                      (0.7, 0.0, 8.0, 0.9, -0.6, 1.5, -2.0)])   # photon, retrograde
-def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph):
+@pytest.mark.parametrize("r_off,h0", [(0.0, 0.0), (0.6, 0.35)])
+def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph, r_off, h0):
     T = 1.0
     y0 = [r0, th0, 0.0, ur, uth, uph]
     errs = []
@@ -380,16 +381,19 @@ def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph):
         # leapfrog (Sec. 3.1): positions live at t_n, velocities at t_(n-1/2).  The oracle starts from
         # x(0) and u(-dt/2) of the brute-force trajectory and must end at x(T), u(T - dt/2) of the same trajectory.
         y_m, y_u, y_x = _brute_force_trace(a, eps, y0, [-0.5 * dt, T - 0.5 * dt, T])
-        g = O.Grid(256, 128, a, 0.9 * (1 + np.sqrt(1 - a * a)), 30.0, n_iter=25)
-        # u_1 = u_r dr/dx1 is the momentum conjugate to x1: its scale factor dxi*r is taken where u lives (t = -dt/2)
-        p = one_particle(O, g, r0, th0, y_m[3] * y_m[0] / r0, y_m[4], y_m[5], massive=int(eps))
+        g = O.Grid(256, 128, a, 0.9 * (1 + np.sqrt(1 - a * a)), 30.0, n_iter=25, r0=r_off, h0=h0)
+        # u_1 = u_r dr/dx1, u_2 = u_theta dtheta/dx2 are the momenta conjugate to x1, x2: their scale factors are
+        # taken where u lives (t = -dt/2), the position where x lives (t = 0)
+        s_m = O.metric(g, *code_position(O, g, y_m[0], y_m[1]), derivs=False)
+        s_0 = O.metric(g, *code_position(O, g, r0, th0), derivs=False)
+        p = one_particle(O, g, r0, th0, y_m[3] * s_m["s1"][0] / s_0["s1"][0], y_m[4] * s_m["s2"][0] / s_0["s2"][0],
+                         y_m[5], massive=int(eps))
         for _ in range(int(round(T / dt))):
             O.push(g, p, None, dt)
         r, th = _phys(O, g, p)
-        dxi, deta = np.log(g.r_max / g.r_min) / g.n1, np.pi / g.n2
-        # covariant u_r at (T - dt/2) in the physical basis: the code-basis scale factor is taken where u lives
-        r_u = y_u[0]
-        got = np.array([r, th, p.phi[0], p.u1[0] / (dxi * r_u), p.u2[0] / deta, p.u3[0]])
+        # covariant components at (T - dt/2) back in the physical basis, scale factors where u lives
+        s_u = O.metric(g, *code_position(O, g, y_u[0], y_u[1]), derivs=False)
+        got = np.array([r, th, p.phi[0], p.u1[0] / s_u["s1"][0], p.u2[0] / s_u["s2"][0], p.u3[0]])
         ref = np.array([y_x[0], y_x[1], y_x[2], y_u[3], y_u[4], y_u[5]])
         errs.append(np.max(np.abs(got - ref) / np.maximum(1.0, np.abs(ref))))
     assert errs[2] < 1e-5, errs                                           # converged to the brute-force trace
