@@ -35,7 +35,7 @@ struct SortState {          // tile table of one species (keyed by the address o
 
 struct grpic_ctx {
   grpic_grid grid;
-  double a, r_min, r_max, small_angle;
+  double a, r_min, r_max, small_angle, r0, h0;
   int n_iter, tile_path, use_tma, early_exit;
   double last_dt;
   bool have_dt;
@@ -78,10 +78,11 @@ Consts<real> make_consts(const grpic_ctx* c) {
   Consts<real> g;
   g.n1 = c->grid.n1; g.n2 = c->grid.n2; g.ng = c->grid.nghost; g.n_iter = c->n_iter;
   g.ld = c->grid.n2 + 2 * c->grid.nghost;
-  const double dxi = std::log(c->r_max / c->r_min) / c->grid.n1;
+  const double dxi = std::log((c->r_max - c->r0) / (c->r_min - c->r0)) / c->grid.n1;
   const double deta = M_PI / c->grid.n2;
   g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
-  g.log_rmin = (real)std::log(c->r_min);
+  g.log_rmin = (real)std::log(c->r_min - c->r0);
+  g.r_off = (real)c->r0; g.h0 = (real)c->h0;
   g.dxi = (real)dxi; g.deta = (real)deta;
   g.inv_dxi = (real)(1.0 / dxi);
   g.inv_deta2 = (real)(1.0 / (deta * deta));
@@ -147,6 +148,7 @@ int check_current(grpic_ctx* ctx, const grpic_current* J, const SpeciesConst& sc
   return GRPIC_OK;
 }
 
+inline bool general_map(const grpic_ctx* c) { return c->r0 != 0.0 || c->h0 != 0.0; }
 inline unsigned grid_for(int64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
 
 int scan_exclusive(grpic_ctx* ctx, uint32_t* d, uint32_t n, cudaStream_t st) {
@@ -202,6 +204,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->grid = *grid;
   ctx->a = a; ctx->r_min = r_min; ctx->r_max = r_max;
   ctx->small_angle = 1e-5;                                  // SMALL_ANGLE_GR
+  ctx->r0 = 0.0; ctx->h0 = 0.0;                             // A.3 map parameters
   ctx->n_iter = 10;
   ctx->tile_path = 1;
   ctx->use_tma = 1;
@@ -270,6 +273,16 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
     ctx->small_angle = v;
     return GRPIC_OK;
   }
+  if (!std::strcmp(key, "r0")) {
+    if (!(v < ctx->r_min)) return fail(ctx, GRPIC_EINVAL, "r0 must be < r_min");
+    ctx->r0 = v;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "h0")) {
+    if (!(v > -0.5 && v < 1.0)) return fail(ctx, GRPIC_EINVAL, "h0 must be in (-0.5, 1): dtheta/deta > 0");
+    ctx->h0 = v;
+    return GRPIC_OK;
+  }
   return fail(ctx, GRPIC_EINVAL, std::string("unknown real key: ") + key);
 }
 
@@ -286,8 +299,12 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
   CK(cudaMemsetAsync(ctx->d_counters, 0, 3 * sizeof(unsigned long long), st));
   if (p->n == 0) return GRPIC_OK;
   JPtrs<real> J{{nullptr, nullptr, nullptr}};
-  k_push_or_step<real, false><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), F, J, sc,
-                                                                 ctx->d_counters);
+  if (general_map(ctx))
+    k_push_or_step<real, false, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), F, J, sc,
+                                                                                   ctx->d_counters);
+  else
+    k_push_or_step<real, false><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), F, J, sc,
+                                                                   ctx->d_counters);
   CK(cudaGetLastError());
   return GRPIC_OK;
 }
@@ -303,7 +320,10 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
   cudaStream_t st = (cudaStream_t)stream;
   CK(cudaMemsetAsync(ctx->d_counters + 3, 0, sizeof(unsigned long long), st));
   if (p->n == 0 || !sc.do_deposit) return GRPIC_OK;
-  k_deposit<real><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters);
+  if (general_map(ctx))
+    k_deposit<real, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters);
+  else
+    k_deposit<real><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters);
   CK(cudaGetLastError());
   return GRPIC_OK;
 }
@@ -327,6 +347,11 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   const PPtrs<real> P = make_pptrs(p);
 
   auto it = ctx->sorted.find((const void*)p->i1);
+  if (general_map(ctx)) {        // full A.3 map (r0, h0): direct kernel with the general coordinate class
+    k_push_or_step<real, true, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    CK(cudaGetLastError());
+    return GRPIC_OK;
+  }
   const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_at_sort <= p->n && sc.em &&
                      sc.do_deposit;
   if (!tiled) {
@@ -551,7 +576,10 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
     UP(P.u1, ph->u1, rb); UP(P.u2, ph->u2, rb); UP(P.u3, ph->u3, rb);
     if (P.phi) UP(P.phi, ph->phi, rb);
     UP(P.w, ph->weight, rb); UP(P.tag, ph->tag, (size_t)m);
-    k_push_or_step<real, true><<<grid_for(m), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    if (general_map(ctx))
+      k_push_or_step<real, true, CoordGen<real>><<<grid_for(m), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    else
+      k_push_or_step<real, true><<<grid_for(m), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
     CK(cudaGetLastError());
     DOWN(ph->i1, P.i1, ib); DOWN(ph->i2, P.i2, ib);
     DOWN(ph->dx1, P.dx1, rb); DOWN(ph->dx2, P.dx2, rb);

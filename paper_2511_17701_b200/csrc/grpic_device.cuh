@@ -36,6 +36,18 @@ struct Consts {
   T th_min, th_max;    // [small_angle, pi - small_angle]
   T sin_min, cos_min;  // sin, cos of th_min
   T sin_max, cos_max;  // sin, cos of th_max (FP64: the values the plain formula gives at the clamped angle)
+  // full A.3 map; both zero in the five BASELINE configs, which then run the specialised Coord<T>
+  T r_off;             // radial offset r0: xi = log(r - r0); log_rmin = log(r_min - r0)
+  T h0;                // polar stretch: theta = eta + 2 h0 eta (pi - 2 eta)(pi - eta)/pi^2
+};
+
+// what the metric at a point needs from the coordinate map besides (r, theta)
+template <typename T>
+struct MapLocal {
+  T rm;        // r - r0            (s1 = dxi*rm)
+  T s2;        // dtheta/dx2 = deta * dtheta/deta
+  T inv_s2sq;  // 1/s2^2
+  T dls2;      // d ln(s2)/dx2
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -166,7 +178,11 @@ struct Coord;
 
 template <>
 struct Coord<double> {
+  static constexpr bool kGeneral = false;
   double x2, r0, th0, s0, c0;
+  __device__ __forceinline__ void local0(const Consts<double>& g, MapLocal<double>& L) const {
+    L.rm = r0; L.s2 = g.deta; L.inv_s2sq = g.inv_deta2; L.dls2 = 0.0;
+  }
   __device__ __forceinline__ void init(const Consts<double>& g, int i1, double dx1, int i2, double dx2) {
     const double x1 = (double)i1 + dx1;
     x2 = (double)i2 + dx2;
@@ -226,6 +242,10 @@ struct Coord<double> {
 
 template <>
 struct Coord<float> {
+  static constexpr bool kGeneral = false;
+  __device__ __forceinline__ void local0(const Consts<float>& g, MapLocal<float>& L) const {
+    L.rm = r0; L.s2 = g.deta; L.inv_s2sq = g.inv_deta2; L.dls2 = 0.f;
+  }
   float r0, thp, s0, c0, sgn;  // r, theta', sin(theta'), cos(theta') at x (theta' unclamped); +1 or -1 (mirrored)
   __device__ __forceinline__ void init(const Consts<float>& g, int i1, float dx1, int i2, float dx2) {
     const float xi = fmaf(dx1, g.dxi, fmaf((float)i1, g.dxi, g.log_rmin));
@@ -293,6 +313,106 @@ struct Coord<float> {
 };
 
 // ------------------------------------------------------------------------------------------------
+// General A.3 map: radial offset r0 and polar stretch h0.  Plain evaluation with the library
+// functions at every point (no polynomial shortcuts): this class serves contexts with r0 != 0 or h0 != 0,
+// the five BASELINE configs run Coord<T> above.  theta(eta) is symmetric about the equator, so FP32 again
+// measures eta from the NEARER axis; FP64 forms x1, x2 and the angle exactly as the plain formulas do.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sincos_(double x, double& s, double& c) { sincos(x, &s, &c); }
+__device__ __forceinline__ void sincos_(float x, float& s, float& c) { sincosf(x, &s, &c); }
+__device__ __forceinline__ double exp_(double x) { return exp(x); }
+__device__ __forceinline__ float exp_(float x) { return expf(x); }
+
+template <typename T>
+struct CoordGen {
+  static constexpr bool kGeneral = true;
+  static constexpr bool kMirror = sizeof(T) == 4;
+  T a1, a2;        // FP64: x1, x2 of x^(n);  FP32: xi and eta' (from the nearer axis) of x^(n)
+  T sgn;           // -1 when mirrored onto the axis theta = pi
+  T r0, rm0, th0, s0, c0, q0;   // at x^(n): r, r - r_off, theta('), sin, cos, dtheta/deta
+
+  __device__ __forceinline__ static T theta_of(const Consts<T>& g, T eta) {
+    if (kMirror) {
+      const T x = eta * T(0.31830988618379067154);                     // eta/pi
+      return eta * fma_(T(2) * g.h0, (T(1) - T(2) * x) * (T(1) - x), T(1));
+    }
+    const T pi = T(3.14159265358979323846);                            // FP64: the plain formula, term by term
+    return eta + T(2) * g.h0 * eta * (pi - T(2) * eta) * (pi - eta) / (pi * pi);
+  }
+  __device__ __forceinline__ static T dtheta_deta(const Consts<T>& g, T eta) {
+    if (kMirror) {
+      const T x = eta * T(0.31830988618379067154);
+      return fma_(T(12) * g.h0, x * (x - T(1)), fma_(T(2), g.h0, T(1)));
+    }
+    const T pi = T(3.14159265358979323846);
+    return T(1) + T(2) * g.h0 + T(12) * g.h0 * (eta / pi) * (eta / pi - T(1));
+  }
+  // (xi, eta or eta') of the point x^(n) + (h1, h2)
+  __device__ __forceinline__ void point(const Consts<T>& g, T h1, T h2, T& xi, T& eta) const {
+    if (kMirror) {
+      xi = fma_(h1, g.dxi, a1);
+      eta = fma_(sgn * g.deta, h2, a2);
+    } else {
+      xi = g.log_rmin + (a1 + h1) * g.dxi;
+      eta = (a2 + h2) * g.deta;
+    }
+  }
+  __device__ __forceinline__ void trig(const Consts<T>& g, T eta, T& sth, T& cth) const {
+    const T th = theta_of(g, eta);
+    T s, c;
+    sincos_(th, s, c);
+    if (kMirror) {
+      if (th < g.th_min) { s = g.sin_min; c = g.cos_min; }
+      c = sgn * c;
+    } else {
+      if (th < g.th_min) { s = g.sin_min; c = g.cos_min; }
+      if (th > g.th_max) { s = g.sin_max; c = g.cos_max; }
+    }
+    sth = s; cth = c;
+  }
+  __device__ __forceinline__ void init(const Consts<T>& g, int i1, T dx1, int i2, T dx2) {
+    sgn = T(1);
+    if (kMirror) {
+      a1 = fma_(dx1, g.dxi, fma_((T)i1, g.dxi, g.log_rmin));
+      const bool upper = 2 * i2 >= g.n2;
+      sgn = upper ? T(-1) : T(1);
+      a2 = ((T)(upper ? g.n2 - i2 : i2) + (upper ? -dx2 : dx2)) * g.deta;
+    } else {
+      a1 = (T)i1 + dx1;
+      a2 = (T)i2 + dx2;
+    }
+    T xi, eta;
+    point(g, T(0), T(0), xi, eta);
+    rm0 = exp_(xi);
+    r0 = g.r_off + rm0;
+    trig(g, eta, s0, c0);
+    q0 = dtheta_deta(g, eta);
+    th0 = eta;
+  }
+  __device__ __forceinline__ void at0(const Consts<T>&, T& r, T& sth, T& cth) const { r = r0; sth = s0; cth = c0; }
+  __device__ __forceinline__ void local0(const Consts<T>& g, MapLocal<T>& L) const {
+    L.rm = rm0;
+    L.s2 = g.deta * q0;
+    L.inv_s2sq = g.inv_deta2 * rcp_(q0 * q0);
+    const T x = th0 * T(0.31830988618379067154);
+    L.dls2 = (sgn * g.deta) * (T(3.8197186342054880585) * g.h0) * (T(2) * x - T(1)) * rcp_(q0);   // 12 h0/pi (2x-1)/q
+  }
+  struct Fast {
+    __device__ __forceinline__ void init(const Consts<T>&, const CoordGen<T>&) {}
+  };
+  // r, r - r_off, 1/(dtheta/deta)^2 and sin(theta) at the midpoint of the displacement (del1, del2)
+  __device__ __forceinline__ void at_mid(const Consts<T>& g, T del1, T del2, T& r, T& rm, T& iq2, T& sth) const {
+    T xi, eta, cth;
+    point(g, T(0.5) * del1, T(0.5) * del2, xi, eta);
+    rm = exp_(xi);
+    r = g.r_off + rm;
+    trig(g, eta, sth, cth);
+    const T q = dtheta_deta(g, eta);
+    iq2 = rcp_(q * q);
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
 // Midpoint evaluation of Eq. 29/30: everything Eq. 29 needs from the metric at (r, sin theta),
 // for a fixed u.  With w1 = u_1/s1, U2 = u_2/s2 (physical-basis covariant components):
 //   G = Sigma gamma^2 = eps Sigma + A w1^2/(Sigma+2r) + U2^2 + u_3^2/sin^2 + 2 a w1 u_3      (Eq. 20)
@@ -346,6 +466,30 @@ struct MidEval {
     R = rsqrt_(Sp2r * G);
     n1 = U.k1 * fma_((t + U.au3) * ir, R, T(-2) * iSp2r);
     n2 = U.k2 * R;
+  }
+  // General A.3 map: s1 = dxi*(r - r0) and s2 = deta*q with q = dtheta/deta at the midpoint (iq2 = 1/q^2).
+  //   beta^1 = 2r/((Sigma+2r) s1),  h^22 = 1/(Sigma s2^2);  the rest as above with 1/r -> 1/(r - r0).
+  __device__ __forceinline__ void eval_gen(const Consts<T>& g, const MidU<T>& U, T r, T rm, T iq2, T sth, T& n1,
+                                           T& n2) {
+    const T s2 = sth * sth;
+    const T a2s2 = U.a2 * s2;
+    const T r2a2 = fma_(r, r, U.a2);
+    const T Sigma = r2a2 - a2s2;
+    const T Sp2r = fma_(T(2), r, Sigma);
+    const T Delta = fma_(r, r - T(2), U.a2);
+    const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
+    const T irm = rcp_(rm);
+    const T iSp2r = rcp_(Sp2r);
+    is2 = rcp_(s2);
+    w1 = U.w1c * irm;
+    const T t = (A * iSp2r) * w1;
+    T G = fma_(U.eps, Sigma, U.U2sq * iq2);
+    G = fma_(t, w1, G);
+    G = fma_(U.u3sq, is2, G);
+    G = fma_(U.c2au3, w1, G);
+    R = rsqrt_(Sp2r * G);
+    n1 = U.k1 * fma_((t + U.au3) * irm, R, (T(-2) * r) * (irm * iSp2r));
+    n2 = (U.k2 * iq2) * R;
   }
   __device__ __forceinline__ T dphidt(const Consts<T>& g, const MidU<T>& U) const {
     return fma_(g.a, w1, U.u3 * is2) * R;
@@ -413,6 +557,60 @@ __device__ __forceinline__ void metric_full(const Consts<T>& g, T r, T sth, T ct
   m.d_beta1[0] = -beta1 * l1P;
   m.d_beta1[1] = -beta1 * l2P;
   const T ka = (iSp2r * iSp2r) * ial;            // 1/((Sigma+2r)^2 alpha)
+  m.d_alpha[0] = fma_(r, d1S, -Sigma * s1) * ka;
+  m.d_alpha[1] = (r * d2S) * ka;
+}
+
+// The same set for the general A.3 map: s1 = dxi (r - r0), s2 = deta dtheta/deta (MapLocal).  Differences:
+//   beta^1 = 2r/((Sigma+2r) s1)  ->  d_1 ln beta^1 = s1/r - dxi - d_1 ln(Sigma+2r);
+//   h^22 = 1/(Sigma s2^2)        ->  d_2 ln h^22 = -d_2 ln Sigma - 2 d_2 ln s2   (the entry P:842 omits);
+//   d_2 Sigma, d_2 A and the cot(theta) term of h^33 carry the local s2.
+template <typename T>
+__device__ __forceinline__ void metric_full_gen(const Consts<T>& g, const MapLocal<T>& L, T r, T sth, T cth,
+                                                MetricFull<T>& m) {
+  const T a = g.a, a2 = g.a2;
+  const T r2 = r * r;
+  const T s2th = sth * sth;
+  const T a2s2 = a2 * s2th;
+  const T r2a2 = r2 + a2;
+  const T Sigma = fma_(a2 * cth, cth, r2);
+  const T Delta = fma_(r, r - T(2), a2);
+  const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
+  const T Sp2r = fma_(T(2), r, Sigma);
+  const T s1 = g.dxi * L.rm;
+  const T iS = rcp_(Sigma), iSp2r = rcp_(Sp2r), is2th = rcp_(s2th);
+  const T is1 = g.inv_dxi * rcp_(L.rm);
+  const T al2 = Sigma * iSp2r;
+  const T ial = rsqrt_(al2);
+  m.alpha = al2 * ial;
+  const T beta1 = ((T(2) * r) * iSp2r) * is1;
+  const T B = (iS * iSp2r) * (is1 * is1);
+  m.hu11 = A * B;
+  m.hu22 = iS * L.inv_s2sq;
+  m.hu33 = iS * is2th;
+  m.hu13 = (a * iS) * is1;
+  m.hd22 = (L.s2 * L.s2) * Sigma;
+  m.hd33 = (A * s2th) * iS;
+  m.hd13 = -(s1 * a) * ((Sp2r * iS) * s2th);
+
+  const T d1S = (T(2) * r) * s1;
+  const T d2S = (T(-2) * a2 * L.s2) * (sth * cth);
+  const T d1A = (T(4) * r * s1) * r2a2 - a2s2 * ((T(2) * (r - T(1))) * s1);
+  const T d2A = d2S * Delta;
+  const T l1S = d1S * iS, l2S = d2S * iS;
+  const T l1P = (d1S + T(2) * s1) * iSp2r;
+  const T l2P = d2S * iSp2r;
+  m.d_hu11[0] = fma_(B, d1A, -m.hu11 * (l1S + l1P + T(2) * g.dxi));
+  m.d_hu11[1] = fma_(B, d2A, -m.hu11 * (l2S + l2P));
+  m.d_hu22[0] = -m.hu22 * l1S;
+  m.d_hu22[1] = -m.hu22 * (l2S + T(2) * L.dls2);
+  m.d_hu33[0] = -m.hu33 * l1S;
+  m.d_hu33[1] = -m.hu33 * fma_((T(2) * L.s2) * cth, rcp_(sth), l2S);
+  m.d_hu13[0] = -m.hu13 * (l1S + g.dxi);
+  m.d_hu13[1] = -m.hu13 * l2S;
+  m.d_beta1[0] = beta1 * (s1 * rcp_(r) - g.dxi - l1P);
+  m.d_beta1[1] = -beta1 * l2P;
+  const T ka = (iSp2r * iSp2r) * ial;
   m.d_alpha[0] = fma_(r, d1S, -Sigma * s1) * ka;
   m.d_alpha[1] = (r * d2S) * ka;
 }
@@ -522,17 +720,23 @@ struct PState {
 
 // returns: 0 alive, 1 absorbed inside (i1 < 0), 2 absorbed outside (i1 >= n1); `dphidt` = Eq. 30 rate;
 // `reflected` tells the caller that the deposited path is not the integrated one.
-template <typename T>
+template <typename T, typename CoordT = Coord<T>>
 __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, bool em, const T Dp[3],
                                              const T Bp[3], T qm, T eps, T dt, T& dphidt, bool& reflected) {
-  Coord<T> X;
+  CoordT X;
   X.init(g, p.i1, p.dx1, p.i2, p.dx2);
   T u[3] = {p.u1, p.u2, p.u3};
   {
     T r, sth, cth;
     X.at0(g, r, sth, cth);
     MetricFull<T> m;
-    metric_full(g, r, sth, cth, m);
+    if constexpr (CoordT::kGeneral) {
+      MapLocal<T> L;
+      X.local0(g, L);
+      metric_full_gen(g, L, r, sth, cth, m);
+    } else {
+      metric_full(g, r, sth, cth, m);
+    }
 
     Tetrad<T> e;
     T cD[3], cB[3], uh[3];
@@ -596,7 +800,25 @@ __device__ __forceinline__ int push_particle(const Consts<T>& g, PState<T>& p, b
   U.init(g, u[0], u[1], u[2], eps, dt);
   MidEval<T> E;
   bool fixed = false;
-  {
+  if constexpr (CoordT::kGeneral) {
+    // general A.3 map: plain evaluation of the map at every midpoint
+    const int n_iter = in_reg(g.n_iter);
+    const bool ee = g.early_exit != 0;
+    for (int it = 0; it < n_iter; ++it) {
+      T r, rm, iq2, sth, n1, n2;
+      X.at_mid(g, del1, del2, r, rm, iq2, sth);
+      E.eval_gen(g, U, r, rm, iq2, sth, n1, n2);
+      fixed = (n1 == del1) & (n2 == del2);
+      del1 = n1;
+      del2 = n2;
+      if (fixed && ee) break;
+    }
+    if (!fixed) {
+      T r, rm, iq2, sth, n1, n2;
+      X.at_mid(g, del1, del2, r, rm, iq2, sth);
+      E.eval_gen(g, U, r, rm, iq2, sth, n1, n2);
+    }
+  } else {
     // fast form: polynomial coordinates, loop constants pinned in registers, no branch but the exit test
     typename Coord<T>::Fast XF;
     XF.init(g, X);
@@ -697,18 +919,24 @@ __device__ __forceinline__ void deposit_segments(int di, int dj, T xa, T ya, T d
 }
 
 // out-of-plane velocity of Eq. 36 at the midpoint of the path (ia + xm, ja + ym), theta clamped
-template <typename T>
+template <typename T, typename CoordT = Coord<T>>
 __device__ __forceinline__ T v3_at_path_midpoint(const Consts<T>& g, int ia, int ja, T xm, T ym, T u1, T u2, T u3,
                                                  T eps) {
-  Coord<T> X;
+  CoordT X;
   X.init(g, ia, xm, ja, ym);
-  T r, sth, cth;
-  X.at0(g, r, sth, cth);
   MidU<T> U;
   U.init(g, u1, u2, u3, eps, T(1));
   MidEval<T> E;
   T n1, n2;
-  E.eval(g, U, r, sth, n1, n2);
+  if constexpr (CoordT::kGeneral) {
+    T r, rm, iq2, sth;
+    X.at_mid(g, T(0), T(0), r, rm, iq2, sth);
+    E.eval_gen(g, U, r, rm, iq2, sth, n1, n2);
+  } else {
+    T r, sth, cth;
+    X.at0(g, r, sth, cth);
+    E.eval(g, U, r, sth, n1, n2);
+  }
   return E.dphidt(g, U);
 }
 

@@ -88,7 +88,7 @@ __device__ __forceinline__ void global_add8(const JPtrs<T>& J, int64_t k, int ld
 // ------------------------------------------------------------------------------------------------
 // shared per-particle driver used by k_push / k_step_direct
 // ------------------------------------------------------------------------------------------------
-template <typename T, bool kDeposit>
+template <typename T, bool kDeposit, typename CoordT = Coord<T>>
 __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                                                 const JPtrs<T>& J, const SpeciesConst& sc,
                                                 unsigned long long* counters, int64_t k) {
@@ -115,7 +115,7 @@ __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<
     const T dt = (T)sc.dt;
     T dphidt;
     bool reflected;
-    res = push_particle(g, p, sc.em != 0, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
+    res = push_particle<T, CoordT>(g, p, sc.em != 0, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
     P.i1[k] = p.i1; P.i2[k] = p.i2; P.dx1[k] = p.dx1; P.dx2[k] = p.dx2;
     P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
     if (sc.has_phi) P.phi[k] += dt * dphidt;
@@ -127,8 +127,8 @@ __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<
       } else {
         T v3 = dphidt;
         if (reflected)
-          v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
-                                   p.u2, p.u3, eps);
+          v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2),
+                                              p.u1, p.u2, p.u3, eps);
         const T qw = (T)sc.charge * P.w[k];
         T seg[2][8];
         deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw / dt, qw, v3, seg);
@@ -150,17 +150,17 @@ __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<
   if (kDeposit) warp_count(counters, 3, over);
 }
 
-template <typename T, bool kDeposit>
+template <typename T, bool kDeposit, typename CoordT = Coord<T>>
 __global__ void __launch_bounds__(kBlock) k_push_or_step(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
                                                          const JPtrs<T> J, const SpeciesConst sc,
                                                          unsigned long long* counters) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  particle_direct<T, kDeposit>(g, P, F, J, sc, counters, k);
+  particle_direct<T, kDeposit, CoordT>(g, P, F, J, sc, counters, k);
 }
 
 // deposit from stored (prev, current) — Eq. 36 velocity recomputed at the path midpoint as the paper
 // states it
-template <typename T>
+template <typename T, typename CoordT = Coord<T>>
 __global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J,
                                                     const SpeciesConst sc, unsigned long long* counters) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPt
     } else {
       const T xa = P.dx1p[k], ya = P.dx2p[k], dx1 = P.dx1[k], dx2 = P.dx2[k];
       const T eps = sc.massive ? T(1) : T(0);
-      const T v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + dx1), T(0.5) * (ya + (T)dj + dx2), P.u1[k],
+      const T v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + dx1), T(0.5) * (ya + (T)dj + dx2), P.u1[k],
                                        P.u2[k], P.u3[k], eps);
       const T qw = (T)sc.charge * P.w[k];
       const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);

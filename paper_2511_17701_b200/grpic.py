@@ -194,7 +194,8 @@ def _stream_ptr(stream):
 class Context:
     """grpic_ctx* with the ABI's calls as methods (same names, same order of arguments)."""
 
-    def __init__(self, n1, n2, a, r_min, r_max, nghost=2, precision="f32", n_iter=None, small_angle=None):
+    def __init__(self, n1, n2, a, r_min, r_max, nghost=2, precision="f32", n_iter=None, small_angle=None,
+                 r0=None, h0=None):
         self.precision = precision
         self.lib = load(precision)
         self.n1, self.n2, self.nghost = int(n1), int(n2), int(nghost)
@@ -208,6 +209,10 @@ class Context:
             self.set_int("n_iter", n_iter)
         if small_angle is not None:
             self.set_real("small_angle", small_angle)
+        if r0 is not None:
+            self.set_real("r0", r0)        # A.3 radial offset
+        if h0 is not None:
+            self.set_real("h0", h0)        # A.3 polar stretch
 
     @property
     def shape(self):
