@@ -347,23 +347,24 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   const PPtrs<real> P = make_pptrs(p);
 
   auto it = ctx->sorted.find((const void*)p->i1);
-  if (general_map(ctx)) {        // full A.3 map (r0, h0): direct kernel with the general coordinate class
-    k_push_or_step<real, true, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
-    CK(cudaGetLastError());
-    return GRPIC_OK;
-  }
   const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_at_sort <= p->n && sc.em &&
                      sc.do_deposit;
+  const bool gen = general_map(ctx);             // full A.3 map (r0, h0): same kernels, general coordinate class
   if (!tiled) {
-    k_push_or_step<real, true><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    if (gen)
+      k_push_or_step<real, true, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
+    else
+      k_push_or_step<real, true><<<grid_for(p->n), kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters);
     CK(cudaGetLastError());
     return GRPIC_OK;
   }
   const SortState& ss = it->second;
   std::string terr;
-  if (!launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items, ss.d_n_items, ss.max_items,
-                               ss.n_at_sort, st, terr))
-    return fail(ctx, GRPIC_ECUDA, terr);
+  const bool ok = gen ? launch_step_tiled<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
+                                                                ss.items, ss.d_n_items, ss.max_items, ss.n_at_sort, st, terr)
+                      : launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
+                                                ss.d_n_items, ss.max_items, ss.n_at_sort, st, terr);
+  if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
   return GRPIC_OK;
 }
 

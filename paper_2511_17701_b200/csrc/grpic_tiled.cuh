@@ -300,7 +300,7 @@ struct RawAcc {      // raw staged stencil: sample (row, col) of component c
   }
 };
 
-template <typename T>
+template <typename T, typename CoordT = Coord<T>>
 __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   // ---- tail blocks: particles appended after the last sort -> direct path ----
   if (blockIdx.x >= max_items) {
     const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
-    particle_direct<T, true>(g, P, F, J, sc, counters, k);
+    particle_direct<T, true, CoordT>(g, P, F, J, sc, counters, k);
     return;
   }
   if (blockIdx.x >= n_items_ptr[0]) return;
@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
       }
       T dphidt;
       bool reflected;
-      const int res = push_particle(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
+      const int res = push_particle<T, CoordT>(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
       P.i1[k] = p.i1; P.i2[k] = p.i2; P.dx1[k] = p.dx1; P.dx2[k] = p.dx2;
       P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
       if (sc.has_phi) P.phi[k] = phi + dt * dphidt;
@@ -444,8 +444,8 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
         } else {
           T v3 = dphidt;
           if (reflected)
-            v3 = v3_at_path_midpoint(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2), p.u1,
-                                     p.u2, p.u3, eps);
+            v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1),
+                                                T(0.5) * (ya + (T)dj + p.dx2), p.u1, p.u2, p.u3, eps);
           const T qw = chg * w;
           deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw * inv_dt, qw, v3, seg);
           const int wb1 = wa1 + di, wb2 = wa2 + dj;
@@ -506,14 +506,14 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   }
 }
 
-template <typename T>
+template <typename T, typename CoordT = Coord<T>>
 bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
                        const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
                        cudaStream_t st, std::string& err) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T, CoordT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)tiled_smem_bytes<T>());
     if (ea != cudaSuccess) {
       err = std::string("k_step_tiled shared-memory opt-in: ") + cudaGetErrorString(ea);
@@ -530,7 +530,7 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   const int nt2 = (g.n2 + kTile - 1) / kTile;
   const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
   const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
-  k_step_tiled<T><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
+  k_step_tiled<T, CoordT><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
                                                                 n_at_sort, nt2, use_tma, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
