@@ -50,6 +50,7 @@ typedef struct {
   double small_angle;    /* SMALL_ANGLE_GR                            */
   double r0;             /* radial offset of A.3: xi = log(r - r0)    */
   double h0;             /* polar stretch of A.3; 0 = uniform     */
+  int32_t linear_r;      /* 1: spherical Kerr-Schild of A.2, r uniform in x1 (r0 unused) */
 } orc_grid;
 
 typedef struct {
@@ -68,6 +69,9 @@ typedef struct {                     /* [0] = d/dx1, [1] = d/dx2              */
 } orc_dmetric_t;
 
 static double orc_dxi(const orc_grid* g) { return log((g->r_max - g->r0) / (g->r_min - g->r0)) / g->n1; }
+/* d ln(s1)/dx1: dxi for s1 = dxi e^xi (A.3), 0 for the constant s1 = dr of A.2 */
+static double orc_dls1(const orc_grid* g) { return g->linear_r ? 0.0 : orc_dxi(g); }
+static double orc_dr(const orc_grid* g) { return (g->r_max - g->r_min) / g->n1; }
 static double orc_deta(const orc_grid* g) { return M_PI / g->n2; }
 
 /* P:820-823 (A.3): xi = log(r - r0) uniform in x1;  eta = x2*deta uniform in x2 and
@@ -82,7 +86,7 @@ static double orc_dtheta_deta(const orc_grid* g, double eta) {
   return 1.0 + 2.0 * g->h0 + 12.0 * g->h0 * (eta / M_PI) * (eta / M_PI - 1.0);
 }
 static void orc_coords(const orc_grid* g, double x1, double x2, double* r, double* th) {
-  *r = g->r0 + exp(log(g->r_min - g->r0) + x1 * orc_dxi(g));
+  *r = g->linear_r ? g->r_min + x1 * orc_dr(g) : g->r0 + exp(log(g->r_min - g->r0) + x1 * orc_dxi(g));
   double t = orc_theta_of_eta(g, x2 * orc_deta(g));
   if (t < g->small_angle) t = g->small_angle;
   if (t > M_PI - g->small_angle) t = M_PI - g->small_angle;
@@ -102,7 +106,7 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
   m->Delta = r * r - 2.0 * r + a * a;
   m->A = (r * r + a * a) * (r * r + a * a) - a * a * m->Delta * s2th;
   m->z = 2.0 * r / m->Sigma;
-  m->s1 = orc_dxi(g) * (r - g->r0);
+  m->s1 = g->linear_r ? orc_dr(g) : orc_dxi(g) * (r - g->r0);
   m->s2 = orc_deta(g) * orc_dtheta_deta(g, x2 * orc_deta(g));
   {
     const double eta = x2 * orc_deta(g);
@@ -128,7 +132,7 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
  * as in A.2. */
 void orc_dmetric(const orc_grid* g, const orc_metric_t* m, orc_dmetric_t* d) {
   const double a = g->a, r = m->r, S = m->Sigma, A = m->A;
-  const double s1 = m->s1, s2 = m->s2, dxi = orc_dxi(g);
+  const double s1 = m->s1, s2 = m->s2, dxi = orc_dls1(g);   /* the A.3 extras vanish on the A.2 map */
   const double sth = m->sth, cth = m->cth, s2th = sth * sth;
   const double d1S = 2.0 * r * s1;
   const double d2S = -2.0 * a * a * sth * cth * s2;

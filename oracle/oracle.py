@@ -32,7 +32,7 @@ def build(force: bool = False) -> str:
 class _Grid(C.Structure):
     _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("ng", C.c_int32), ("n_iter", C.c_int32),
                 ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double),
-                ("r0", C.c_double), ("h0", C.c_double)]
+                ("r0", C.c_double), ("h0", C.c_double), ("linear_r", C.c_int32)]
 
 
 _METRIC_NAMES = ["r", "th", "sth", "cth", "Sigma", "Delta", "A", "z", "s1", "s2", "alpha", "beta1",
@@ -83,10 +83,11 @@ class Grid:
     small_angle: float = 1e-5
     r0: float = 0.0          # A.3 radial offset, xi = log(r - r0)
     h0: float = 0.0          # A.3 polar stretch
+    linear_r: int = 0        # 1: A.2 map, r uniform in x1
 
     def c(self) -> _Grid:
         return _Grid(self.n1, self.n2, self.ng, self.n_iter, self.a, self.r_min, self.r_max, self.small_angle,
-                     self.r0, self.h0)
+                     self.r0, self.h0, self.linear_r)
 
     @property
     def shape(self):

@@ -23,8 +23,11 @@ def code_position(O, g, r, theta):
     """(x1, x2) of physical (r, theta) under the A.3 map of grid g (r0, h0 may be non-zero): the radial map is
     inverted in closed form, the polar one by bisection on the oracle's own theta(x2)."""
     r0, h0 = getattr(g, "r0", 0.0), getattr(g, "h0", 0.0)
-    dxi = np.log((g.r_max - r0) / (g.r_min - r0)) / g.n1
-    x1 = np.log((r - r0) / (g.r_min - r0)) / dxi
+    if getattr(g, "linear_r", 0):
+        x1 = (r - g.r_min) / ((g.r_max - g.r_min) / g.n1)
+    else:
+        dxi = np.log((g.r_max - r0) / (g.r_min - r0)) / g.n1
+        x1 = np.log((r - r0) / (g.r_min - r0)) / dxi
     if h0 == 0.0:
         return x1, theta / (np.pi / g.n2)
     lo, hi = 0.0, float(g.n2)

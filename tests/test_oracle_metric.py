@@ -6,12 +6,14 @@ import pytest
 PTS = [(3.2, 7.9), (60.5, 31.7), (100.1, 3.3), (10.0, 60.2), (120.9, 32.0)]
 
 
-@pytest.fixture(scope="module", params=["log_uniform", "offset_stretched"])
+@pytest.fixture(scope="module", params=["log_uniform", "offset_stretched", "linear_r"])
 def g(O, request):
     """The map of the five configs (A.3 with r0 = 0, h0 = 0) and the full A.3 map: radial offset
     r0 = 0.6 and polar stretch h0 = 0.35; every pin below that does not name the map holds for both."""
     if request.param == "log_uniform":
         return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0)
+    if request.param == "linear_r":                     # spherical Kerr-Schild of App. A.2 (P:800-816)
+        return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0, linear_r=1)
     return O.Grid(128, 64, 0.95, 0.9 * (1 + np.sqrt(1 - 0.95 ** 2)), 20.0, r0=0.6, h0=0.35)
 
 
@@ -56,8 +58,9 @@ def test_schwarzschild_limit(O):
 
 def test_coordinate_map(O, g):
     m = O.metric(g, np.array([0.0, 128.0, 64.0]), np.array([32.0, 32.0, 16.0]))
-    # xi = log(r - r0) is uniform in x1: the middle of the grid is the geometric mean of (r - r0)
-    assert np.allclose(m["r"], [g.r_min, g.r_max, g.r0 + np.sqrt((g.r_min - g.r0) * (g.r_max - g.r0))], rtol=1e-14)
+    # xi = log(r - r0) is uniform in x1: the middle of the grid is the geometric mean of (r - r0); A.2: the arithmetic mean
+    mid = 0.5 * (g.r_min + g.r_max) if g.linear_r else g.r0 + np.sqrt((g.r_min - g.r0) * (g.r_max - g.r0))
+    assert np.allclose(m["r"], [g.r_min, g.r_max, mid], rtol=1e-14)
     # theta(eta) of P:821 at eta = pi/2 and pi/4: pi/2 (fixed point of the stretch) and pi/4 + 2 h0 (pi/4)(pi/2)(3pi/4)/pi^2
     assert np.allclose(m["th"], [np.pi / 2, np.pi / 2, np.pi / 4 * (1 + 0.75 * g.h0)], rtol=1e-14)
 

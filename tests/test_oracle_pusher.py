@@ -372,8 +372,8 @@ def _brute_force_trace(a, eps, y0, times):
 @pytest.mark.parametrize("a,eps,r0,th0,ur,uth,uph", [(0.9, 1.0, 6.0, 1.2, -0.1, 0.8, 2.5),      # inclined bound-ish orbit
                                                      (0.995, 1.0, 3.0, np.pi / 2 - 0.3, 0.05, -0.5, 1.9),  # near the hole
                                                      (0.7, 0.0, 8.0, 0.9, -0.6, 1.5, -2.0)])   # photon, retrograde
-@pytest.mark.parametrize("r_off,h0", [(0.0, 0.0), (0.6, 0.35)])
-def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph, r_off, h0):
+@pytest.mark.parametrize("r_off,h0,lin", [(0.0, 0.0, 0), (0.6, 0.35, 0), (0.0, 0.0, 1)])
+def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph, r_off, h0, lin):
     T = 1.0
     y0 = [r0, th0, 0.0, ur, uth, uph]
     errs = []
@@ -381,7 +381,7 @@ def test_brute_force_single_particle_trace(O, a, eps, r0, th0, ur, uth, uph, r_o
         # leapfrog (Sec. 3.1): positions live at t_n, velocities at t_(n-1/2).  The oracle starts from
         # x(0) and u(-dt/2) of the brute-force trajectory and must end at x(T), u(T - dt/2) of the same trajectory.
         y_m, y_u, y_x = _brute_force_trace(a, eps, y0, [-0.5 * dt, T - 0.5 * dt, T])
-        g = O.Grid(256, 128, a, 0.9 * (1 + np.sqrt(1 - a * a)), 30.0, n_iter=25, r0=r_off, h0=h0)
+        g = O.Grid(256, 128, a, 0.9 * (1 + np.sqrt(1 - a * a)), 30.0, n_iter=25, r0=r_off, h0=h0, linear_r=lin)
         # u_1 = u_r dr/dx1, u_2 = u_theta dtheta/dx2 are the momenta conjugate to x1, x2: their scale factors are
         # taken where u lives (t = -dt/2), the position where x lives (t = 0)
         s_m = O.metric(g, *code_position(O, g, y_m[0], y_m[1]), derivs=False)
