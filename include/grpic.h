@@ -61,7 +61,8 @@ typedef struct grpic_ctx grpic_ctx; /* opaque, library-owned */
 /* The mesh: n1 = N_r, n2 = N_theta cells, nghost >= 1 ghost layers on every side. */
 typedef struct {
   int32_t n1, n2, nghost;
-  int32_t r_map; /* 1 = logarithmic r (App. A.3, r0 = 0, h0 = 0). Only 1 is built. */
+  int32_t r_map; /* 1 = logarithmic r (quasi-spherical map of App. A.3; "r0", "h0" via grpic_set_real);
+                    0 = uniform r (spherical Kerr-Schild of App. A.2: r = r_min + x1 (r_max - r_min)/n1) */
 } grpic_grid;
 
 /* One species, structure-of-arrays.
@@ -91,7 +92,7 @@ int grpic_real_bytes(void);
 /* Create a context for one mesh and one Kerr spin a (|a| <= 1), radial extent [r_min, r_max]
  * in units of r_g (north_star: grpic_create(grid, a, r_min, r_max); metric of App. A.3).
  * Defaults: n_iter = 10, small_angle = 1e-5 (SMALL_ANGLE_GR).
- * Errors: EINVAL (NULL, n1/n2 < 1, nghost < 1, r_map != 1, r_min <= 0 or >= r_max), ECUDA, ENOMEM. */
+ * Errors: EINVAL (NULL, n1/n2 < 1, nghost < 1, r_map not 0 or 1, r_min <= 0 or >= r_max), ECUDA, ENOMEM. */
 int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, grpic_ctx** out);
 int grpic_destroy(grpic_ctx* ctx);
 

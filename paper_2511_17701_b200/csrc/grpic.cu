@@ -78,10 +78,15 @@ Consts<real> make_consts(const grpic_ctx* c) {
   Consts<real> g;
   g.n1 = c->grid.n1; g.n2 = c->grid.n2; g.ng = c->grid.nghost; g.n_iter = c->n_iter;
   g.ld = c->grid.n2 + 2 * c->grid.nghost;
-  const double dxi = std::log((c->r_max - c->r0) / (c->r_min - c->r0)) / c->grid.n1;
+  const bool lin = c->grid.r_map == 0;             // A.2: dxi = 1 and rm = dr make s1 = dxi*rm = dr (grpic_device.cuh)
+  const double dxi = lin ? 1.0 : std::log((c->r_max - c->r0) / (c->r_min - c->r0)) / c->grid.n1;
   const double deta = M_PI / c->grid.n2;
+  g.r_lin = lin ? 1 : 0;
+  g.r_min = (real)c->r_min;
+  g.dr = (real)((c->r_max - c->r_min) / c->grid.n1);
+  g.dls1 = lin ? (real)0 : (real)dxi;
   g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
-  g.log_rmin = (real)std::log(c->r_min - c->r0);
+  g.log_rmin = lin ? (real)0 : (real)std::log(c->r_min - c->r0);
   g.r_off = (real)c->r0; g.h0 = (real)c->h0;
   g.dxi = (real)dxi; g.deta = (real)deta;
   g.inv_dxi = (real)(1.0 / dxi);
@@ -148,7 +153,7 @@ int check_current(grpic_ctx* ctx, const grpic_current* J, const SpeciesConst& sc
   return GRPIC_OK;
 }
 
-inline bool general_map(const grpic_ctx* c) { return c->r0 != 0.0 || c->h0 != 0.0; }
+inline bool general_map(const grpic_ctx* c) { return c->r0 != 0.0 || c->h0 != 0.0 || c->grid.r_map == 0; }
 inline unsigned grid_for(int64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
 
 int scan_exclusive(grpic_ctx* ctx, uint32_t* d, uint32_t n, cudaStream_t st) {
@@ -190,7 +195,8 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   *out = nullptr;
   if (grid->n1 < 1 || grid->n2 < 1) return fail(nullptr, GRPIC_EINVAL, "n1, n2 must be >= 1");
   if (grid->nghost < 1) return fail(nullptr, GRPIC_EINVAL, "nghost must be >= 1 (the gather reads one ghost layer)");
-  if (grid->r_map != 1) return fail(nullptr, GRPIC_EINVAL, "only r_map = 1 (logarithmic r, App. A.3) is built");
+  if (grid->r_map != 0 && grid->r_map != 1)
+    return fail(nullptr, GRPIC_EINVAL, "r_map must be 1 (logarithmic r, App. A.3) or 0 (uniform r, App. A.2)");
   if (!(r_min > 0.0) || !(r_max > r_min)) return fail(nullptr, GRPIC_EINVAL, "need 0 < r_min < r_max");
   if (!(std::fabs(a) <= 1.0)) return fail(nullptr, GRPIC_EINVAL, "need |a| <= 1");
   if ((int64_t)(grid->n1 + 2 * grid->nghost) * (grid->n2 + 2 * grid->nghost) > 0x7fffffffll)

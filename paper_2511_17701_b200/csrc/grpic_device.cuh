@@ -39,6 +39,10 @@ struct Consts {
   // full A.3 map; both zero in the five BASELINE configs, which then run the specialised Coord<T>
   T r_off;             // radial offset r0: xi = log(r - r0); log_rmin = log(r_min - r0)
   T h0;                // polar stretch: theta = eta + 2 h0 eta (pi - 2 eta)(pi - eta)/pi^2
+  // spherical Kerr-Schild map of A.2: r = r_min + x1*dr.  Then dxi = inv_dxi = 1 and rm = dr, so that
+  // s1 = dxi*rm = dr everywhere below, and dls1 = d ln(s1)/dx1 = 0 (A.3: dls1 = dxi)
+  int32_t r_lin;
+  T r_min, dr, dls1;
 };
 
 // what the metric at a point needs from the coordinate map besides (r, theta)
@@ -347,15 +351,20 @@ struct CoordGen {
     const T pi = T(3.14159265358979323846);
     return T(1) + T(2) * g.h0 + T(12) * g.h0 * (eta / pi) * (eta / pi - T(1));
   }
-  // (xi, eta or eta') of the point x^(n) + (h1, h2)
+  // (xi, eta or eta') of the point x^(n) + (h1, h2); on the A.2 map "xi" is r itself
   __device__ __forceinline__ void point(const Consts<T>& g, T h1, T h2, T& xi, T& eta) const {
     if (kMirror) {
-      xi = fma_(h1, g.dxi, a1);
+      xi = fma_(h1, g.r_lin ? g.dr : g.dxi, a1);
       eta = fma_(sgn * g.deta, h2, a2);
     } else {
-      xi = g.log_rmin + (a1 + h1) * g.dxi;
+      xi = g.r_lin ? g.r_min + (a1 + h1) * g.dr : g.log_rmin + (a1 + h1) * g.dxi;
       eta = (a2 + h2) * g.deta;
     }
+  }
+  // r and r - r_off (A.3) or r and dr (A.2) from the radial coordinate of point()
+  __device__ __forceinline__ void radius(const Consts<T>& g, T xi, T& r, T& rm) const {
+    if (g.r_lin) { r = xi; rm = g.dr; }
+    else { rm = exp_(xi); r = g.r_off + rm; }
   }
   __device__ __forceinline__ void trig(const Consts<T>& g, T eta, T& sth, T& cth) const {
     const T th = theta_of(g, eta);
@@ -373,7 +382,7 @@ struct CoordGen {
   __device__ __forceinline__ void init(const Consts<T>& g, int i1, T dx1, int i2, T dx2) {
     sgn = T(1);
     if (kMirror) {
-      a1 = fma_(dx1, g.dxi, fma_((T)i1, g.dxi, g.log_rmin));
+      a1 = g.r_lin ? fma_(dx1, g.dr, fma_((T)i1, g.dr, g.r_min)) : fma_(dx1, g.dxi, fma_((T)i1, g.dxi, g.log_rmin));
       const bool upper = 2 * i2 >= g.n2;
       sgn = upper ? T(-1) : T(1);
       a2 = ((T)(upper ? g.n2 - i2 : i2) + (upper ? -dx2 : dx2)) * g.deta;
@@ -383,8 +392,7 @@ struct CoordGen {
     }
     T xi, eta;
     point(g, T(0), T(0), xi, eta);
-    rm0 = exp_(xi);
-    r0 = g.r_off + rm0;
+    radius(g, xi, r0, rm0);
     trig(g, eta, s0, c0);
     q0 = dtheta_deta(g, eta);
     th0 = eta;
@@ -404,8 +412,7 @@ struct CoordGen {
   __device__ __forceinline__ void at_mid(const Consts<T>& g, T del1, T del2, T& r, T& rm, T& iq2, T& sth) const {
     T xi, eta, cth;
     point(g, T(0.5) * del1, T(0.5) * del2, xi, eta);
-    rm = exp_(xi);
-    r = g.r_off + rm;
+    radius(g, xi, r, rm);
     trig(g, eta, sth, cth);
     const T q = dtheta_deta(g, eta);
     iq2 = rcp_(q * q);
@@ -600,15 +607,15 @@ __device__ __forceinline__ void metric_full_gen(const Consts<T>& g, const MapLoc
   const T l1S = d1S * iS, l2S = d2S * iS;
   const T l1P = (d1S + T(2) * s1) * iSp2r;
   const T l2P = d2S * iSp2r;
-  m.d_hu11[0] = fma_(B, d1A, -m.hu11 * (l1S + l1P + T(2) * g.dxi));
+  m.d_hu11[0] = fma_(B, d1A, -m.hu11 * (l1S + l1P + T(2) * g.dls1));
   m.d_hu11[1] = fma_(B, d2A, -m.hu11 * (l2S + l2P));
   m.d_hu22[0] = -m.hu22 * l1S;
   m.d_hu22[1] = -m.hu22 * (l2S + T(2) * L.dls2);
   m.d_hu33[0] = -m.hu33 * l1S;
   m.d_hu33[1] = -m.hu33 * fma_((T(2) * L.s2) * cth, rcp_(sth), l2S);
-  m.d_hu13[0] = -m.hu13 * (l1S + g.dxi);
+  m.d_hu13[0] = -m.hu13 * (l1S + g.dls1);
   m.d_hu13[1] = -m.hu13 * l2S;
-  m.d_beta1[0] = beta1 * (s1 * rcp_(r) - g.dxi - l1P);
+  m.d_beta1[0] = beta1 * (s1 * rcp_(r) - g.dls1 - l1P);
   m.d_beta1[1] = -beta1 * l2P;
   const T ka = (iSp2r * iSp2r) * ial;
   m.d_alpha[0] = fma_(r, d1S, -Sigma * s1) * ka;

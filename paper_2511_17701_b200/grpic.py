@@ -195,11 +195,11 @@ class Context:
     """grpic_ctx* with the ABI's calls as methods (same names, same order of arguments)."""
 
     def __init__(self, n1, n2, a, r_min, r_max, nghost=2, precision="f32", n_iter=None, small_angle=None,
-                 r0=None, h0=None):
+                 r0=None, h0=None, r_map=1):
         self.precision = precision
         self.lib = load(precision)
         self.n1, self.n2, self.nghost = int(n1), int(n2), int(nghost)
-        g = _Grid(self.n1, self.n2, self.nghost, 1)
+        g = _Grid(self.n1, self.n2, self.nghost, int(r_map))
         h = _vp()
         rc = self.lib.grpic_create(C.byref(g), float(a), float(r_min), float(r_max), C.byref(h))
         if rc != GRPIC_OK:

@@ -190,14 +190,15 @@ def test_ragged_grids_ghost_widths_iteration_counts(G, O, W, n1, n2, ng, n_iter,
 
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])
-@pytest.mark.parametrize("r0,h0", [(0.6, 0.0), (0.0, 0.35), (0.5, -0.3)])
-def test_general_a3_map(G, O, W, prec, r0, h0):
+@pytest.mark.parametrize("r0,h0,lin", [(0.6, 0.0, 0), (0.0, 0.35, 0), (0.5, -0.3, 0), (0.0, 0.0, 1), (0.0, 0.4, 1)])
+def test_general_a3_map(G, O, W, prec, r0, h0, lin):
     """Full map of App. A.3: radial offset r0 and polar stretch h0.  The oracle's map is
     pinned by finite differences and brute-force traces (test_oracle_*); here the general-map kernels against it:
     split and fused paths, charged particles in smooth random fields, 4 steps."""
     a, n1, n2, ng = 0.9, 96, 48, 2
-    g = O.Grid(n1, n2, a, 0.9 * W.horizon_radius(a), 30.0, ng=ng, r0=r0, h0=h0)
-    rng = np.random.Generator(np.random.Philox(int(1000 * r0 + 100 * (h0 + 1))))
+    # lin = 1: the uniform-r map of App. A.2 (r_map = 0), here also combined with the polar stretch
+    g = O.Grid(n1, n2, a, 0.9 * W.horizon_radius(a), 12.0 if lin else 30.0, ng=ng, r0=r0, h0=h0, linear_r=lin)
+    rng = np.random.Generator(np.random.Philox(int(1000 * r0 + 100 * (h0 + 1)) + lin))
     shape = (n1 + 2 * ng, n2 + 2 * ng)
     ii, jj = np.meshgrid(np.arange(shape[0]), np.arange(shape[1]), indexing="ij")
     fields = {k: 0.3 * np.sin(0.21 * ii + p) * np.cos(0.17 * jj - p) + 0.05 * rng.uniform(-1, 1, shape)
@@ -220,7 +221,7 @@ def test_general_a3_map(G, O, W, prec, r0, h0):
         sp.u1, sp.u2, sp.u3 = uh[0] * m["s1"], uh[1] * m["s2"] * m["r"], uh[2] * m["r"] * m["sth"]
         sp.weight = rng.random(n) + 0.5; sp.tag = np.ones(n, np.uint8); sp.phi = np.zeros(n)
         sp.q_over_m, sp.charge, sp.massive = q, q, 1
-        ctx = G.Context(n1, n2, a, g.r_min, g.r_max, nghost=ng, precision=prec, r0=r0, h0=h0)
+        ctx = G.Context(n1, n2, a, g.r_min, g.r_max, nghost=ng, precision=prec, r0=r0, h0=h0, r_map=0 if lin else 1)
         names = ("D1", "D2", "D3", "B1", "B2", "B3")
         fdev = G.grid_tensors(fields, names, prec)
         fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
@@ -229,7 +230,7 @@ def test_general_a3_map(G, O, W, prec, r0, h0):
             ctx.sort(ps)                                  # a sorted species must still take the general-map kernels
             for step in range(4):
                 res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode)
-        print("A.3 map", r0, h0, prec, q, res, c)
+        print("map", "A.2" if lin else "A.3", r0, h0, prec, q, res, c)
 
 
 def test_sort_is_a_permutation_into_key_order(G, O, W):
