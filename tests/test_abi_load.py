@@ -51,7 +51,7 @@ def test_create_validates_arguments_and_never_falls_back(libs):
     assert b"n1" in lib.grpic_last_error(None)
     g = grpic._Grid(8, 8, 0, 1)
     assert lib.grpic_create(C.byref(g), 0.9, 1.0, 20.0, C.byref(h)) == grpic.GRPIC_EINVAL
-    g = grpic._Grid(8, 8, 2, 0)
+    g = grpic._Grid(8, 8, 2, 2)          # r_map: 1 = A.3 (log r), 0 = A.2 (uniform r); anything else is refused
     assert lib.grpic_create(C.byref(g), 0.9, 1.0, 20.0, C.byref(h)) == grpic.GRPIC_EINVAL
     g = grpic._Grid(8, 8, 2, 1)
     assert lib.grpic_create(C.byref(g), 0.9, 20.0, 1.0, C.byref(h)) == grpic.GRPIC_EINVAL
