@@ -51,6 +51,8 @@ typedef struct {
   double r0;             /* radial offset of A.3: xi = log(r - r0)    */
   double h0;             /* polar stretch of A.3; 0 = uniform     */
   int32_t linear_r;      /* 1: spherical Kerr-Schild of A.2, r uniform in x1 (r0 unused) */
+  double mass;           /* M in units of r_g: 1 everywhere in the paper's GR runs; 0 with a = 0 is the flat
+                            spherical metric kerr_schild_0 of A.1: z = 0, alpha = 1, beta = 0          */
 } orc_grid;
 
 typedef struct {
@@ -98,14 +100,14 @@ static void orc_coords(const orc_grid* g, double x1, double x2, double* r, doubl
 void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
   double r, th;
   orc_coords(g, x1, x2, &r, &th);
-  const double a = g->a;
+  const double a = g->a, M = g->mass;
   m->r = r; m->th = th;
   m->sth = sin(th); m->cth = cos(th);
   const double s2th = m->sth * m->sth;
   m->Sigma = r * r + a * a * m->cth * m->cth;
-  m->Delta = r * r - 2.0 * r + a * a;
+  m->Delta = r * r - 2.0 * M * r + a * a;
   m->A = (r * r + a * a) * (r * r + a * a) - a * a * m->Delta * s2th;
-  m->z = 2.0 * r / m->Sigma;
+  m->z = 2.0 * M * r / m->Sigma;
   m->s1 = g->linear_r ? orc_dr(g) : orc_dxi(g) * (r - g->r0);
   m->s2 = orc_deta(g) * orc_dtheta_deta(g, x2 * orc_deta(g));
   {
@@ -114,7 +116,7 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
   }
   m->alpha = 1.0 / sqrt(1.0 + m->z);
   m->beta1 = m->z / (1.0 + m->z) / m->s1;
-  m->hu11 = m->A / (m->Sigma * (m->Sigma + 2.0 * r)) / (m->s1 * m->s1);
+  m->hu11 = m->A / (m->Sigma * (m->Sigma + 2.0 * M * r)) / (m->s1 * m->s1);
   m->hu22 = 1.0 / m->Sigma / (m->s2 * m->s2);
   m->hu33 = 1.0 / (m->Sigma * s2th);
   m->hu13 = a / m->Sigma / m->s1;
@@ -131,30 +133,30 @@ void orc_metric(const orc_grid* g, double x1, double x2, orc_metric_t* m) {
  * printed text (DESIGN.md R-S2): d_theta Sigma from P:774; sign of d_xi alpha
  * as in A.2. */
 void orc_dmetric(const orc_grid* g, const orc_metric_t* m, orc_dmetric_t* d) {
-  const double a = g->a, r = m->r, S = m->Sigma, A = m->A;
+  const double a = g->a, M = g->mass, r = m->r, S = m->Sigma, A = m->A;   /* M = 1: the printed A.2 list */
   const double s1 = m->s1, s2 = m->s2, dxi = orc_dls1(g);   /* the A.3 extras vanish on the A.2 map */
   const double sth = m->sth, cth = m->cth, s2th = sth * sth;
   const double d1S = 2.0 * r * s1;
   const double d2S = -2.0 * a * a * sth * cth * s2;
-  const double d1D = 2.0 * (r - 1.0) * s1;
+  const double d1D = 2.0 * (r - M) * s1;
   const double d1A = 4.0 * r * s1 * (r * r + a * a) - a * a * s2th * d1D;
   const double d2A = -2.0 * a * a * sth * cth * m->Delta * s2;
-  const double den = S * S * (S + 2.0 * r) * (S + 2.0 * r);
+  const double den = S * S * (S + 2.0 * M * r) * (S + 2.0 * M * r);
 
-  d->hu11[0] = (S * (S + 2.0 * r) * d1A - 2.0 * A * (r * d1S + S * (d1S + s1))) / den / (s1 * s1)
+  d->hu11[0] = (S * (S + 2.0 * M * r) * d1A - 2.0 * A * (M * r * d1S + S * (d1S + M * s1))) / den / (s1 * s1)
                - 2.0 * dxi * m->hu11;
-  d->hu11[1] = (S * (S + 2.0 * r) * d2A - 2.0 * A * d2S * (r + S)) / den / (s1 * s1);
+  d->hu11[1] = (S * (S + 2.0 * M * r) * d2A - 2.0 * A * d2S * (M * r + S)) / den / (s1 * s1);
   d->hu22[0] = -d1S / (S * S) / (s2 * s2);
   d->hu22[1] = -d2S / (S * S) / (s2 * s2) - 2.0 * m->dls2 * m->hu22;   /* A.3: s2 depends on x2 */
   d->hu33[0] = -d1S / (S * S * s2th);
   d->hu33[1] = -2.0 * cth * s2 / (S * S * sth * s2th) * (S - a * a * s2th);
   d->hu13[0] = -a / s1 * d1S / (S * S) - dxi * m->hu13;
   d->hu13[1] = -a / s1 * d2S / (S * S);
-  d->beta1[0] = 2.0 / s1 * (s1 * S - r * d1S) / ((S + 2.0 * r) * (S + 2.0 * r)) - dxi * m->beta1;
-  d->beta1[1] = -2.0 / s1 * r * d2S / (S * S * (1.0 + m->z) * (1.0 + m->z));
+  d->beta1[0] = 2.0 * M / s1 * (s1 * S - r * d1S) / ((S + 2.0 * M * r) * (S + 2.0 * M * r)) - dxi * m->beta1;
+  d->beta1[1] = -2.0 * M / s1 * r * d2S / (S * S * (1.0 + m->z) * (1.0 + m->z));
   const double al3 = m->alpha * m->alpha * m->alpha;
-  d->alpha[0] = -(s1 * S - r * d1S) / (S * S) * al3;
-  d->alpha[1] = r * d2S / (S * S) * al3;
+  d->alpha[0] = -M * (s1 * S - r * d1S) / (S * S) * al3;
+  d->alpha[1] = M * r * d2S / (S * S) * al3;
 }
 
 /* Tetrads, matrix form of P:754 (the explicit inverse formulas at P:766/770

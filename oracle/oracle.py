@@ -32,7 +32,8 @@ def build(force: bool = False) -> str:
 class _Grid(C.Structure):
     _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("ng", C.c_int32), ("n_iter", C.c_int32),
                 ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double),
-                ("r0", C.c_double), ("h0", C.c_double), ("linear_r", C.c_int32)]
+                ("r0", C.c_double), ("h0", C.c_double), ("linear_r", C.c_int32),
+                ("mass", C.c_double)]
 
 
 _METRIC_NAMES = ["r", "th", "sth", "cth", "Sigma", "Delta", "A", "z", "s1", "s2", "alpha", "beta1",
@@ -84,10 +85,11 @@ class Grid:
     r0: float = 0.0          # A.3 radial offset, xi = log(r - r0)
     h0: float = 0.0          # A.3 polar stretch
     linear_r: int = 0        # 1: A.2 map, r uniform in x1
+    mass: float = 1.0        # M/r_g; 0 (with a = 0) = flat spherical kerr_schild_0 of A.1
 
     def c(self) -> _Grid:
         return _Grid(self.n1, self.n2, self.ng, self.n_iter, self.a, self.r_min, self.r_max, self.small_angle,
-                     self.r0, self.h0, self.linear_r)
+                     self.r0, self.h0, self.linear_r, self.mass)
 
     @property
     def shape(self):

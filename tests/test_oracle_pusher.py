@@ -461,3 +461,68 @@ def test_brute_force_charged_trace_in_wald_field(O, W):
         errs.append(np.max(np.abs(got - ref) / np.maximum(1.0, np.abs(ref))))
     assert errs[2] < 1e-5, errs
     assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
+
+
+# ------------------------------------------------------------------ flat spherical metric (App. A.1) and the SR-EM row
+def _flat_grid(O, n=256, n_iter=10):
+    return O.Grid(n, n, 0.0, 1.0, 20.0, linear_r=1, mass=0.0, n_iter=n_iter)
+
+
+def test_flat_metric_is_appendix_a1(O):
+    """kerr_schild_0: h_ij = diag(dr^2, dtheta^2 r^2, r^2 sin^2), alpha = 1, beta = 0,
+    sqrt(h) = dr dtheta r^2 sin(theta); every derivative vanishes except the three the paper prints."""
+    g = _flat_grid(O)
+    x1 = np.array([3.3, 100.7, 200.2]); x2 = np.array([20.4, 128.0, 230.9])
+    m = O.metric(g, x1, x2)
+    dr, dth = (g.r_max - g.r_min) / g.n1, np.pi / g.n2
+    r, th = g.r_min + x1 * dr, x2 * dth
+    assert np.allclose(m["r"], r, rtol=1e-15) and np.allclose(m["th"], th, rtol=1e-15)
+    assert np.all(m["alpha"] == 1.0) and np.all(m["beta1"] == 0.0) and np.all(m["hd13"] == 0.0) and np.all(m["hu13"] == 0.0)
+    assert np.allclose(m["hd11"], dr ** 2, rtol=1e-14) and np.allclose(m["hd22"], (dth * r) ** 2, rtol=1e-14)
+    assert np.allclose(m["hd33"], (r * np.sin(th)) ** 2, rtol=1e-14)
+    assert np.allclose(m["sqrt_h"], dr * dth * r ** 2 * np.sin(th), rtol=1e-14)
+    assert np.allclose(m["d1_hu33"], -dr * 2 / (r ** 3 * np.sin(th) ** 2), rtol=1e-13)
+    assert np.allclose(m["d1_hu22"], -dr * 2 / (r ** 3 * dth ** 2), rtol=1e-13)
+    assert np.allclose(m["d2_hu33"], -2 * dth * np.cos(th) / (r ** 2 * np.sin(th) ** 3), rtol=1e-13)
+    for k in ("d1_hu11", "d2_hu11", "d2_hu22", "d1_hu13", "d2_hu13", "d1_alpha", "d2_alpha", "d1_beta1", "d2_beta1"):
+        assert np.all(m[k] == 0.0), k
+
+
+def test_table1_sr_em_gyration_closed_orbit(O):
+    """SR-EM row of Table 1: flat metric, uniform vertical field, rho0 = 2 r_g.  Textbook
+    gyration: E = sqrt(2) (printed 1.41421), and the orbit is the circle of Larmor radius
+    rho = rho0 * u_phi-hat = 2 r_g that closes after T = 2 pi gamma/(qB/m); "the trajectory remains closed
+    and the energy error stays bounded".  The curvilinear inertial terms of Eq. 26-29 and the tetrad
+    projections must cancel to leave a circle in the plane."""
+    row = table1()["SR-EM"]
+    g = _flat_grid(O, 1024)
+    qB = 2 * row["Bn"]                                                   # q B0/m with q/m = 1
+    p = one_particle(O, g, row["r"], row["theta"], row["u1"], 0.0, row["u3"], q_over_m=1.0)
+    gam0 = np.sqrt(1 + (row["u3"] / row["r"]) ** 2)
+    assert abs(gam0 - row["E"]) < 1e-5                                    # printed energy
+    dt = row["dt"]
+    T = 2 * np.pi * gam0 / qB
+    n = int(round(T / dt))
+    xs, ys, gs = [], [], []
+    for _ in range(n):
+        m = O.metric(g, *pos(p), derivs=False)
+        r, th = m["r"][0], m["th"][0]
+        B = [qB * np.cos(th) / m["s1"][0], -qB * np.sin(th) / (r * m["s2"][0]), 0.0]   # uniform B0 z-hat, code basis
+        xa = pos(p)
+        O.push_given_fields(g, p, [0.0, 0.0, 0.0], B, dt)
+        xb = pos(p)
+        m = O.metric(g, *xb, derivs=False)
+        r = m["r"][0]
+        xs.append(r * np.cos(p.phi[0])); ys.append(r * np.sin(p.phi[0]))
+        mm = O.metric(g, 0.5 * (xa[0] + xb[0]), 0.5 * (xa[1] + xb[1]), derivs=False)   # P:585: position at the velocity time level
+        gs.append(np.sqrt(1 + mm["hu11"][0] * p.u1[0] ** 2 + mm["hu22"][0] * p.u2[0] ** 2 + mm["hu33"][0] * p.u3[0] ** 2))
+        assert abs(m["th"][0] - np.pi / 2) < 1e-12                        # stays in the equatorial plane
+    xs, ys, gs = np.array(xs), np.array(ys), np.array(gs)
+    assert np.max(np.abs(gs / gam0 - 1)) < 1e-6                           # bounded energy error (P:623)
+    cx, cy = xs.mean(), ys.mean()
+    rho = np.hypot(xs - cx, ys - cy)
+    # gyro-centre 2 r_g from the start point; the printed u is used as u(-dt/2) (leapfrog), which shifts the circle by
+    # v dt/2 = 0.0035 r_g along the initial velocity
+    assert abs(abs(cx - row["r"]) - 2.0) < 2e-3 and abs(cy) < 6e-3
+    assert np.max(np.abs(rho - 2.0)) < 2e-3                               # Larmor radius rho = 2 r_g
+    assert np.hypot(xs[-1] - row["r"], ys[-1]) < 2e-2                     # closed after one period (n*dt ~ T)
