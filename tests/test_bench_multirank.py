@@ -20,7 +20,7 @@ ms, units = bench.reduce_over_ranks(10.0 + 5.0 * rank, 1000 * (rank + 1), dist.g
 assert ms == 15.0 and units == 3000.0, (ms, units)
 dist.barrier()
 dist.destroy_process_group()
-print("ok", rank)
+open(os.path.join(os.environ["GRPIC_OUT"], f"rank{rank}.ok"), "w").write("ok")
 """
 
 
@@ -33,12 +33,12 @@ def _free_port():
 def test_reduce_over_ranks_gloo_world2(tmp_path):
     w = tmp_path / "worker.py"
     w.write_text(_WORKER)
-    env = dict(os.environ, GRPIC_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
+    env = dict(os.environ, GRPIC_ROOT=ROOT, GRPIC_OUT=str(tmp_path), MASTER_ADDR="127.0.0.1")
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
            "--master-port", str(_free_port()), str(w)]
     r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stdout + r.stderr
-    assert "ok 0" in r.stdout and "ok 1" in r.stdout
+    assert (tmp_path / "rank0.ok").exists() and (tmp_path / "rank1.ok").exists()   # both ranks passed their asserts
 
 
 def test_reference_arm_runs_on_rank0_only():
