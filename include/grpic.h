@@ -109,7 +109,9 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t value);
  * "r0", "h0":    the remaining parameters of the quasi-spherical map of App. A.3, both 0 by default:
  *                xi = log(r - r0) uniform in x1 (r0 < r_min; r_min, r_max keep their meaning), and
  *                theta = eta + 2 h0 eta (pi - 2 eta)(pi - eta)/pi^2 with eta = x2*pi/n2 (-0.5 < h0 < 1).
- *                With either non-zero every call runs the same kernels instantiated with the general coordinate
+ * "mass":        M in units of r_g, default 1.  0 together with a = 0 gives the flat spherical metric
+ *                kerr_schild_0 of App. A.1 that the paper uses for its SR-EM test.
+ *                With any of these off its default every call runs the same kernels instantiated with the general coordinate
  *                class (plain evaluation of the map at every point instead of the default map's shortcuts). */
 int grpic_set_real(grpic_ctx* ctx, const char* key, double value);
 

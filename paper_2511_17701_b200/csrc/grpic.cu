@@ -35,7 +35,7 @@ struct SortState {          // tile table of one species (keyed by the address o
 
 struct grpic_ctx {
   grpic_grid grid;
-  double a, r_min, r_max, small_angle, r0, h0;
+  double a, r_min, r_max, small_angle, r0, h0, mass;
   int n_iter, tile_path, use_tma, early_exit;
   double last_dt;
   bool have_dt;
@@ -87,7 +87,7 @@ Consts<real> make_consts(const grpic_ctx* c) {
   g.dls1 = lin ? (real)0 : (real)dxi;
   g.a = (real)c->a; g.a2 = (real)(c->a * c->a);
   g.log_rmin = lin ? (real)0 : (real)std::log(c->r_min - c->r0);
-  g.r_off = (real)c->r0; g.h0 = (real)c->h0;
+  g.r_off = (real)c->r0; g.h0 = (real)c->h0; g.mass = (real)c->mass;
   g.dxi = (real)dxi; g.deta = (real)deta;
   g.inv_dxi = (real)(1.0 / dxi);
   g.inv_deta2 = (real)(1.0 / (deta * deta));
@@ -153,7 +153,9 @@ int check_current(grpic_ctx* ctx, const grpic_current* J, const SpeciesConst& sc
   return GRPIC_OK;
 }
 
-inline bool general_map(const grpic_ctx* c) { return c->r0 != 0.0 || c->h0 != 0.0 || c->grid.r_map == 0; }
+inline bool general_map(const grpic_ctx* c) {
+  return c->r0 != 0.0 || c->h0 != 0.0 || c->grid.r_map == 0 || c->mass != 1.0;
+}
 inline unsigned grid_for(int64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
 
 int scan_exclusive(grpic_ctx* ctx, uint32_t* d, uint32_t n, cudaStream_t st) {
@@ -211,6 +213,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->a = a; ctx->r_min = r_min; ctx->r_max = r_max;
   ctx->small_angle = 1e-5;                                  // SMALL_ANGLE_GR
   ctx->r0 = 0.0; ctx->h0 = 0.0;                             // A.3 map parameters
+  ctx->mass = 1.0;                                          // r_g = M = 1
   ctx->n_iter = 10;
   ctx->tile_path = 1;
   ctx->use_tma = 1;
@@ -282,6 +285,11 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
   if (!std::strcmp(key, "r0")) {
     if (!(v < ctx->r_min)) return fail(ctx, GRPIC_EINVAL, "r0 must be < r_min");
     ctx->r0 = v;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "mass")) {
+    if (!(v >= 0.0)) return fail(ctx, GRPIC_EINVAL, "mass must be >= 0");
+    ctx->mass = v;
     return GRPIC_OK;
   }
   if (!std::strcmp(key, "h0")) {

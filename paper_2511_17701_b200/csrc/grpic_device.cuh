@@ -43,6 +43,9 @@ struct Consts {
   // s1 = dxi*rm = dr everywhere below, and dls1 = d ln(s1)/dx1 = 0 (A.3: dls1 = dxi)
   int32_t r_lin;
   T r_min, dr, dls1;
+  // M in units of r_g (1 in the paper's GR runs); M = 0 with a = 0 is the flat kerr_schild_0 metric of A.1.
+  // Only the general-map functions read it; Coord<T> / metric_full / eval have M = 1 folded in.
+  T mass;
 };
 
 // what the metric at a point needs from the coordinate map besides (r, theta)
@@ -482,8 +485,9 @@ struct MidEval {
     const T a2s2 = U.a2 * s2;
     const T r2a2 = fma_(r, r, U.a2);
     const T Sigma = r2a2 - a2s2;
-    const T Sp2r = fma_(T(2), r, Sigma);
-    const T Delta = fma_(r, r - T(2), U.a2);
+    const T M2 = T(2) * g.mass;
+    const T Sp2r = fma_(M2, r, Sigma);
+    const T Delta = fma_(r, r - M2, U.a2);
     const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
     const T irm = rcp_(rm);
     const T iSp2r = rcp_(Sp2r);
@@ -495,7 +499,7 @@ struct MidEval {
     G = fma_(U.u3sq, is2, G);
     G = fma_(U.c2au3, w1, G);
     R = rsqrt_(Sp2r * G);
-    n1 = U.k1 * fma_((t + U.au3) * irm, R, (T(-2) * r) * (irm * iSp2r));
+    n1 = U.k1 * fma_((t + U.au3) * irm, R, (-M2 * r) * (irm * iSp2r));
     n2 = (U.k2 * iq2) * R;
   }
   __device__ __forceinline__ T dphidt(const Consts<T>& g, const MidU<T>& U) const {
@@ -575,22 +579,22 @@ __device__ __forceinline__ void metric_full(const Consts<T>& g, T r, T sth, T ct
 template <typename T>
 __device__ __forceinline__ void metric_full_gen(const Consts<T>& g, const MapLocal<T>& L, T r, T sth, T cth,
                                                 MetricFull<T>& m) {
-  const T a = g.a, a2 = g.a2;
+  const T a = g.a, a2 = g.a2, M = g.mass;
   const T r2 = r * r;
   const T s2th = sth * sth;
   const T a2s2 = a2 * s2th;
   const T r2a2 = r2 + a2;
   const T Sigma = fma_(a2 * cth, cth, r2);
-  const T Delta = fma_(r, r - T(2), a2);
+  const T Delta = fma_(r, r - T(2) * M, a2);
   const T A = fma_(-a2s2, Delta, r2a2 * r2a2);
-  const T Sp2r = fma_(T(2), r, Sigma);
+  const T Sp2r = fma_(T(2) * M, r, Sigma);
   const T s1 = g.dxi * L.rm;
   const T iS = rcp_(Sigma), iSp2r = rcp_(Sp2r), is2th = rcp_(s2th);
   const T is1 = g.inv_dxi * rcp_(L.rm);
   const T al2 = Sigma * iSp2r;
   const T ial = rsqrt_(al2);
   m.alpha = al2 * ial;
-  const T beta1 = ((T(2) * r) * iSp2r) * is1;
+  const T beta1 = ((T(2) * M * r) * iSp2r) * is1;
   const T B = (iS * iSp2r) * (is1 * is1);
   m.hu11 = A * B;
   m.hu22 = iS * L.inv_s2sq;
@@ -602,10 +606,10 @@ __device__ __forceinline__ void metric_full_gen(const Consts<T>& g, const MapLoc
 
   const T d1S = (T(2) * r) * s1;
   const T d2S = (T(-2) * a2 * L.s2) * (sth * cth);
-  const T d1A = (T(4) * r * s1) * r2a2 - a2s2 * ((T(2) * (r - T(1))) * s1);
+  const T d1A = (T(4) * r * s1) * r2a2 - a2s2 * ((T(2) * (r - M)) * s1);
   const T d2A = d2S * Delta;
   const T l1S = d1S * iS, l2S = d2S * iS;
-  const T l1P = (d1S + T(2) * s1) * iSp2r;
+  const T l1P = (d1S + T(2) * M * s1) * iSp2r;
   const T l2P = d2S * iSp2r;
   m.d_hu11[0] = fma_(B, d1A, -m.hu11 * (l1S + l1P + T(2) * g.dls1));
   m.d_hu11[1] = fma_(B, d2A, -m.hu11 * (l2S + l2P));
@@ -618,8 +622,8 @@ __device__ __forceinline__ void metric_full_gen(const Consts<T>& g, const MapLoc
   m.d_beta1[0] = beta1 * (s1 * rcp_(r) - g.dls1 - l1P);
   m.d_beta1[1] = -beta1 * l2P;
   const T ka = (iSp2r * iSp2r) * ial;
-  m.d_alpha[0] = fma_(r, d1S, -Sigma * s1) * ka;
-  m.d_alpha[1] = (r * d2S) * ka;
+  m.d_alpha[0] = (M * fma_(r, d1S, -Sigma * s1)) * ka;
+  m.d_alpha[1] = (M * r * d2S) * ka;
 }
 
 // ------------------------------------------------------------------------------------------------

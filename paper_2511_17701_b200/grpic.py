@@ -195,7 +195,7 @@ class Context:
     """grpic_ctx* with the ABI's calls as methods (same names, same order of arguments)."""
 
     def __init__(self, n1, n2, a, r_min, r_max, nghost=2, precision="f32", n_iter=None, small_angle=None,
-                 r0=None, h0=None, r_map=1):
+                 r0=None, h0=None, r_map=1, mass=None):
         self.precision = precision
         self.lib = load(precision)
         self.n1, self.n2, self.nghost = int(n1), int(n2), int(nghost)
@@ -213,6 +213,8 @@ class Context:
             self.set_real("r0", r0)        # A.3 radial offset
         if h0 is not None:
             self.set_real("h0", h0)        # A.3 polar stretch
+        if mass is not None:
+            self.set_real("mass", mass)    # 0 with a = 0: flat kerr_schild_0 (App. A.1)
 
     @property
     def shape(self):

@@ -190,14 +190,15 @@ def test_ragged_grids_ghost_widths_iteration_counts(G, O, W, n1, n2, ng, n_iter,
 
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])
-@pytest.mark.parametrize("r0,h0,lin", [(0.6, 0.0, 0), (0.0, 0.35, 0), (0.5, -0.3, 0), (0.0, 0.0, 1), (0.0, 0.4, 1)])
-def test_general_a3_map(G, O, W, prec, r0, h0, lin):
+@pytest.mark.parametrize("r0,h0,lin,mass", [(0.6, 0.0, 0, 1.0), (0.0, 0.35, 0, 1.0), (0.5, -0.3, 0, 1.0), (0.0, 0.0, 1, 1.0),
+                                            (0.0, 0.4, 1, 1.0), (0.0, 0.0, 1, 0.0)])
+def test_general_a3_map(G, O, W, prec, r0, h0, lin, mass):
     """Full map of App. A.3: radial offset r0 and polar stretch h0.  The oracle's map is
     pinned by finite differences and brute-force traces (test_oracle_*); here the general-map kernels against it:
     split and fused paths, charged particles in smooth random fields, 4 steps."""
-    a, n1, n2, ng = 0.9, 96, 48, 2
+    a, n1, n2, ng = (0.9 if mass else 0.0), 96, 48, 2      # mass = 0, a = 0: flat kerr_schild_0 of App. A.1
     # lin = 1: the uniform-r map of App. A.2 (r_map = 0), here also combined with the polar stretch
-    g = O.Grid(n1, n2, a, 0.9 * W.horizon_radius(a), 12.0 if lin else 30.0, ng=ng, r0=r0, h0=h0, linear_r=lin)
+    g = O.Grid(n1, n2, a, 0.9 * W.horizon_radius(a), 12.0 if lin else 30.0, ng=ng, r0=r0, h0=h0, linear_r=lin, mass=mass)
     rng = np.random.Generator(np.random.Philox(int(1000 * r0 + 100 * (h0 + 1)) + lin))
     shape = (n1 + 2 * ng, n2 + 2 * ng)
     ii, jj = np.meshgrid(np.arange(shape[0]), np.arange(shape[1]), indexing="ij")
@@ -221,7 +222,7 @@ def test_general_a3_map(G, O, W, prec, r0, h0, lin):
         sp.u1, sp.u2, sp.u3 = uh[0] * m["s1"], uh[1] * m["s2"] * m["r"], uh[2] * m["r"] * m["sth"]
         sp.weight = rng.random(n) + 0.5; sp.tag = np.ones(n, np.uint8); sp.phi = np.zeros(n)
         sp.q_over_m, sp.charge, sp.massive = q, q, 1
-        ctx = G.Context(n1, n2, a, g.r_min, g.r_max, nghost=ng, precision=prec, r0=r0, h0=h0, r_map=0 if lin else 1)
+        ctx = G.Context(n1, n2, a, g.r_min, g.r_max, nghost=ng, precision=prec, r0=r0, h0=h0, r_map=0 if lin else 1, mass=mass)
         names = ("D1", "D2", "D3", "B1", "B2", "B3")
         fdev = G.grid_tensors(fields, names, prec)
         fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
