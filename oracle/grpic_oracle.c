@@ -516,3 +516,166 @@ void orc_set_num_threads(int n) {
   (void)n;
 #endif
 }
+
+/* ========================================================================
+ * Field-solver half: auxiliary fields Eq. 38/42-44,
+ * Faraday Eq. 40, Ampere Eq. 41 with the polar-axis
+ * update of D^1 Eq. 45 (polar area P:792-794).
+ * Plain loops over the mesh; arrays [n1+2G][n2+2G] as above; ghost ROWS (i < 0,
+ * i >= n1) of the inputs are the caller's, ghost COLUMNS beyond the
+ * axes are not read.  Rows updated: every row whose x1-stencils lie inside the
+ * arrays (aux: array rows 1..rows-2; Faraday/Ampere: array rows 2..rows-3).
+ * Readings (DESIGN.md R-F*): Eq. 44 is garbled in the text; every <.> is the
+ * two-point volume-weighted average along x1 of Eq. 43, written with
+ * sqrt(h~) = sqrt(h)/sin(theta) so that the axis rows are regular.
+ * The metric here is NOT clamped at the axis (sin(theta) = 0 there, exactly).
+ * ====================================================================== */
+typedef struct { double alpha, h11, h22, h33, h13, sqh_t, beta1, sth; } orc_fm;   /* sqh_t = sqrt(h)/sin(theta) */
+
+static void orc_field_metric(const orc_grid* g, double x1, double x2, orc_fm* f) {
+  orc_grid gg = *g;
+  gg.small_angle = 0.0;
+  orc_metric_t m;
+  orc_metric(&gg, x1, x2, &m);
+  /* exactly on the axes sin(theta) must be exactly 0 (x2 = 0) or the rounded sin(pi) made 0 (x2 = n2) */
+  double sth = m.sth;
+  if (x2 == 0.0 || x2 == (double)g->n2) sth = 0.0;
+  const double s2th = sth * sth;
+  f->alpha = m.alpha;
+  f->h11 = m.hd11;
+  f->h22 = m.hd22;
+  f->h33 = m.A * s2th / m.Sigma;
+  f->h13 = -m.s1 * g->a * (1.0 + m.z) * s2th;
+  f->sqh_t = m.s1 * m.s2 * m.Sigma / m.alpha;
+  f->beta1 = m.beta1;
+  f->sth = sth;
+}
+
+#define ORC_AT(F, a1, a2) (F)[(int64_t)(a1) * ld + (a2)]
+
+/* E_i at the D^i locations, H_i at the B^i locations (Eq. 42).  Any output pointer may be NULL. */
+void orc_aux_fields(const orc_grid* g, const orc_fields* F, double* E1, double* E2, double* E3,
+                    double* H1, double* H2, double* H3) {
+  const int G = g->ng, rows = g->n1 + 2 * G;
+  const int64_t ld = g->n2 + 2 * G;
+  for (int a1 = 1; a1 < rows - 1; ++a1) {
+    const double i = (double)(a1 - G);
+    for (int j = 0; j <= g->n2; ++j) {
+      const int a2 = j + G;
+      const double x2 = (double)j;
+      orc_fm c, l, r, cl, cr;   /* centre and the two x1-neighbours of each interpolation */
+      /* ---- locations with integer j: E1 (i+1/2,j), E3 (i,j), H2 (i+1/2,j) ---- */
+      orc_field_metric(g, i + 0.5, x2, &c);
+      orc_field_metric(g, i, x2, &l);
+      orc_field_metric(g, i + 1.0, x2, &r);
+      if (E1) {
+        const double avg = (l.sqh_t * l.h13 * ORC_AT(F->D3, a1, a2) + r.sqh_t * r.h13 * ORC_AT(F->D3, a1 + 1, a2))
+                           / (2.0 * c.sqh_t);
+        ORC_AT(E1, a1, a2) = c.alpha * (c.h11 * ORC_AT(F->D1, a1, a2) + avg);
+      }
+      if (H2) {
+        const double avg = 0.5 * (l.sqh_t * l.sth * l.beta1 * ORC_AT(F->D3, a1, a2)
+                                  + r.sqh_t * r.sth * r.beta1 * ORC_AT(F->D3, a1 + 1, a2));
+        ORC_AT(H2, a1, a2) = c.alpha * c.h22 * ORC_AT(F->B2, a1, a2) + avg;
+      }
+      if (E3) {
+        orc_field_metric(g, i - 0.5, x2, &cl);
+        const double a13 = (cl.sqh_t * cl.h13 * ORC_AT(F->D1, a1 - 1, a2) + c.sqh_t * c.h13 * ORC_AT(F->D1, a1, a2))
+                           / (2.0 * l.sqh_t);
+        const double ab = 0.5 * (cl.sqh_t * cl.sth * cl.beta1 * ORC_AT(F->B2, a1 - 1, a2)
+                                 + c.sqh_t * c.sth * c.beta1 * ORC_AT(F->B2, a1, a2));
+        ORC_AT(E3, a1, a2) = l.alpha * (l.h33 * ORC_AT(F->D3, a1, a2) + a13) + ab;
+      }
+      if (j == g->n2) continue;
+      /* ---- locations with half-integer j: E2 (i,j+1/2), H1 (i,j+1/2), H3 (i+1/2,j+1/2) ---- */
+      orc_field_metric(g, i, x2 + 0.5, &c);
+      orc_field_metric(g, i - 0.5, x2 + 0.5, &cl);
+      orc_field_metric(g, i + 0.5, x2 + 0.5, &cr);
+      if (E2) {
+        const double ab = 0.5 * (cl.sqh_t * cl.sth * cl.beta1 * ORC_AT(F->B3, a1 - 1, a2)
+                                 + cr.sqh_t * cr.sth * cr.beta1 * ORC_AT(F->B3, a1, a2));
+        ORC_AT(E2, a1, a2) = c.alpha * c.h22 * ORC_AT(F->D2, a1, a2) - ab;
+      }
+      if (H1) {
+        const double a13 = (cl.sqh_t * cl.h13 * ORC_AT(F->B3, a1 - 1, a2) + cr.sqh_t * cr.h13 * ORC_AT(F->B3, a1, a2))
+                           / (2.0 * c.sqh_t);
+        ORC_AT(H1, a1, a2) = c.alpha * (c.h11 * ORC_AT(F->B1, a1, a2) + a13);
+      }
+      if (H3) {
+        orc_field_metric(g, i + 1.0, x2 + 0.5, &r);
+        const double a13 = (c.sqh_t * c.h13 * ORC_AT(F->B1, a1, a2) + r.sqh_t * r.h13 * ORC_AT(F->B1, a1 + 1, a2))
+                           / (2.0 * cr.sqh_t);
+        const double ab = 0.5 * (c.sqh_t * c.sth * c.beta1 * ORC_AT(F->D2, a1, a2)
+                                 + r.sqh_t * r.sth * r.beta1 * ORC_AT(F->D2, a1 + 1, a2));
+        ORC_AT(H3, a1, a2) = cr.alpha * (cr.h33 * ORC_AT(F->B3, a1, a2) + a13) - ab;
+      }
+    }
+  }
+}
+
+static double orc_sqrt_h(const orc_grid* g, double x1, double x2) {
+  orc_fm f;
+  orc_field_metric(g, x1, x2, &f);
+  return f.sqh_t * f.sth;
+}
+
+/* Eq. 40: B^i -= dt e^{ijk} d_j E_k with 1/sqrt(h) at the component's own location.
+ * B^2 on the two axes is not evolved. */
+void orc_faraday(const orc_grid* g, double* B1, double* B2, double* B3, const double* E1, const double* E2,
+                 const double* E3, double dt) {
+  const int G = g->ng, rows = g->n1 + 2 * G;
+  const int64_t ld = g->n2 + 2 * G;
+  for (int a1 = 2; a1 < rows - 2; ++a1) {
+    const double i = (double)(a1 - G);
+    for (int j = 0; j < g->n2; ++j) {
+      const int a2 = j + G;
+      ORC_AT(B1, a1, a2) -= dt * (ORC_AT(E3, a1, a2 + 1) - ORC_AT(E3, a1, a2)) / orc_sqrt_h(g, i, j + 0.5);
+      if (j > 0)
+        ORC_AT(B2, a1, a2) += dt * (ORC_AT(E3, a1 + 1, a2) - ORC_AT(E3, a1, a2)) / orc_sqrt_h(g, i + 0.5, (double)j);
+      ORC_AT(B3, a1, a2) -= dt * ((ORC_AT(E2, a1 + 1, a2) - ORC_AT(E2, a1, a2))
+                                  - (ORC_AT(E1, a1, a2 + 1) - ORC_AT(E1, a1, a2))) / orc_sqrt_h(g, i + 0.5, j + 0.5);
+    }
+  }
+}
+
+/* Polar area with a half-cell radius around the axis (P:792-794 for A.1, P:810-812 for A.2; the A.3 form follows with
+ * dr -> s1 and the stretched theta): A_{i+1/2} = int_0^{1/2} sqrt(h) dx2 = s1 (r^2+a^2) sqrt(1 + 2Mr/(r^2+a^2)) (1 - cos theta(1/2)) */
+static double orc_polar_area(const orc_grid* g, double x1) {
+  orc_grid gg = *g;
+  gg.small_angle = 0.0;
+  orc_metric_t m;
+  orc_metric(&gg, x1, 0.5, &m);
+  const double q = m.r * m.r + g->a * g->a;
+  return m.s1 * q * sqrt(1.0 + 2.0 * g->mass * m.r / q) * (1.0 - cos(m.th));
+}
+
+/* Eq. 41: D^i += dt (e^{ijk} d_j H_k - kJ J^i)/sqrt(h), J = deposited conformal currents (may be NULL),
+ * kJ = 4 pi in the paper's Gaussian form.  On the axes D^3 is not evolved and D^1 takes the integral form Eq. 45:
+ * D^1 += dt (+-H_3 of the neighbouring half cell - (kJ/2) J^1)/A_{i+1/2}, sign + at theta = 0 and - at theta = pi
+ * (the circulation around the polar cap reverses; reading R-F2). */
+void orc_ampere(const orc_grid* g, double* D1, double* D2, double* D3, const double* H1, const double* H2,
+                const double* H3, const double* J1, const double* J2, const double* J3, double kJ, double dt) {
+  const int G = g->ng, rows = g->n1 + 2 * G;
+  const int64_t ld = g->n2 + 2 * G;
+  for (int a1 = 2; a1 < rows - 2; ++a1) {
+    const double i = (double)(a1 - G);
+    for (int j = 0; j <= g->n2; ++j) {
+      const int a2 = j + G;
+      const double j1 = J1 ? ORC_AT(J1, a1, a2) : 0.0;
+      if (j == 0)
+        ORC_AT(D1, a1, a2) += dt * (ORC_AT(H3, a1, a2) - 0.5 * kJ * j1) / orc_polar_area(g, i + 0.5);
+      else if (j == g->n2)
+        ORC_AT(D1, a1, a2) += dt * (-ORC_AT(H3, a1, a2 - 1) - 0.5 * kJ * j1) / orc_polar_area(g, i + 0.5);
+      else
+        ORC_AT(D1, a1, a2) += dt * ((ORC_AT(H3, a1, a2) - ORC_AT(H3, a1, a2 - 1)) - kJ * j1) / orc_sqrt_h(g, i + 0.5, (double)j);
+      if (j == g->n2) continue;
+      const double j2 = J2 ? ORC_AT(J2, a1, a2) : 0.0;
+      ORC_AT(D2, a1, a2) += dt * (-(ORC_AT(H3, a1, a2) - ORC_AT(H3, a1 - 1, a2)) - kJ * j2) / orc_sqrt_h(g, i, j + 0.5);
+      if (j > 0) {
+        const double j3 = J3 ? ORC_AT(J3, a1, a2) : 0.0;
+        ORC_AT(D3, a1, a2) += dt * ((ORC_AT(H2, a1, a2) - ORC_AT(H2, a1 - 1, a2))
+                                    - (ORC_AT(H1, a1, a2) - ORC_AT(H1, a1, a2 - 1)) - kJ * j3) / orc_sqrt_h(g, i, (double)j);
+      }
+    }
+  }
+}

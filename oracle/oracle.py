@@ -250,6 +250,54 @@ def deposit(g: Grid, p: Particles, dt: float, J=None):
     return J, int(over.value)
 
 
+# ----------------------------------------------------------------------------------------------
+# Field-solver half: Eq. 42-44 auxiliary fields, Eq. 40 Faraday, Eq. 41/45 Ampere
+# ----------------------------------------------------------------------------------------------
+def _grid_arr(g, a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    assert a.shape == g.shape
+    return a
+
+
+def aux_fields(g: Grid, fields: dict) -> dict:
+    """E1,E2,E3 (at the D^i locations) and H1,H2,H3 (at the B^i locations) from D^i, B^i."""
+    f = {k: _grid_arr(g, fields[k]) for k in ("D1", "D2", "D3", "B1", "B2", "B3")}
+    fc = _Fields(*[_ptr(f[k], _dp) for k in ("D1", "D2", "D3", "B1", "B2", "B3")])
+    out = {k: np.zeros(g.shape) for k in ("E1", "E2", "E3", "H1", "H2", "H3")}
+    gc = g.c()
+    lib().orc_aux_fields(C.byref(gc), C.byref(fc), *[_ptr(out[k], _dp) for k in ("E1", "E2", "E3", "H1", "H2", "H3")])
+    return out
+
+
+def faraday(g: Grid, B: dict, E: dict, dt: float) -> dict:
+    """B^i updated in place (dict B1,B2,B3 of float64 arrays) with E_i; returns B."""
+    for k in ("B1", "B2", "B3"):
+        assert B[k].dtype == np.float64 and B[k].flags.c_contiguous and B[k].shape == g.shape
+    gc = g.c()
+    lib().orc_faraday(C.byref(gc), *[_ptr(B[k], _dp) for k in ("B1", "B2", "B3")],
+                      *[_ptr(_grid_arr(g, E[k]), _dp) for k in ("E1", "E2", "E3")], C.c_double(dt))
+    return B
+
+
+def ampere(g: Grid, D: dict, H: dict, J, dt: float, kJ: float = 4.0 * np.pi) -> dict:
+    """D^i updated in place with H_i and the conformal currents J (dict or None); returns D."""
+    for k in ("D1", "D2", "D3"):
+        assert D[k].dtype == np.float64 and D[k].flags.c_contiguous and D[k].shape == g.shape
+    Hs = [_grid_arr(g, H[k]) for k in ("H1", "H2", "H3")]
+    Js = [None] * 3 if J is None else [_grid_arr(g, J[k]) for k in ("J1", "J2", "J3")]
+    gc = g.c()
+    lib().orc_ampere(C.byref(gc), *[_ptr(D[k], _dp) for k in ("D1", "D2", "D3")], *[_ptr(h, _dp) for h in Hs],
+                     *[None if j is None else _ptr(j, _dp) for j in Js], C.c_double(kJ), C.c_double(dt))
+    return D
+
+
+def sqrt_h(g: Grid, x1, x2):
+    """sqrt(h) at arbitrary code positions, axis not clamped (field side)."""
+    gg = Grid(g.n1, g.n2, g.a, g.r_min, g.r_max, g.ng, g.n_iter, 0.0, g.r0, g.h0, g.linear_r, g.mass)
+    m = metric(gg, x1, x2, derivs=False)
+    return m["sqrt_h"]
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 
