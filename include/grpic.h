@@ -154,6 +154,27 @@ int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_absorbed_in, int
  * the numerator of the throughput metric.  Synchronises `cuda_stream`. */
 int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* cuda_stream);
 
+/* ---- Field-solver half of the step (Sec. 3.3).  Grid kernels; same array layout; device pointers. ----
+ * The caller sequences them and the time levels (Sec. 3.4) and fills the ghost ROWS i < 0, i >= n1 of the inputs
+ * (P:461-467); ghost columns beyond the axes are not read.  Rows written: every row whose x1-stencil lies inside the
+ * arrays (aux: array rows 1 .. rows-2; Faraday/Ampere: array rows 2 .. rows-3; with nghost = 2 that is the whole mesh).
+ * The metric at every Yee location is evaluated in FP64 in both builds. */
+typedef struct { grpic_real *F1, *F2, *F3; } grpic_vec3;
+
+/* Auxiliary fields (Eq. 38, 42-44): E_i = alpha h_ij D^j + e_ijk beta^j B^k at the D^i locations and
+ * H_i = alpha h_ij B^j - e_ijk beta^j D^k at the B^i locations; components at other Yee locations are brought over by
+ * the two-point volume-weighted average along x1 (Eq. 43) written with sqrt(h)/sin(theta).
+ * E or H may be NULL (only the other is computed).  Errors: EINVAL, ECUDA. */
+int grpic_aux_fields(grpic_ctx* ctx, const grpic_fields* em, grpic_vec3* E, grpic_vec3* H, void* cuda_stream);
+
+/* Faraday (Eq. 40): B^i -= dt e^{ijk} d_j E_k / sqrt(h), B^2 on the axes untouched. */
+int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt, void* cuda_stream);
+
+/* Ampere (Eq. 41): D^i += dt (e^{ijk} d_j H_k - k_J J^i)/sqrt(h) with the deposited conformal currents J (may be NULL);
+ * k_J = 4 pi unless changed with grpic_set_real("k_J").  D^3 on the axes untouched; D^1 on the axes by the integral
+ * form Eq. 45 with the polar area of App. A. */
+int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic_current* J, double dt, void* cuda_stream);
+
 /* End-to-end convenience: every pointer in p, fields and J is HOST memory (pinned or pageable).
  * Copies fields and particle columns to library-owned device buffers in chunks, runs the fused step
  * chunk by chunk (copies overlapped with compute on two streams), accumulates J on the device and

@@ -16,6 +16,7 @@
 #include "../../include/grpic.h"
 #include "grpic_kernels.cuh"
 #include "grpic_tiled.cuh"
+#include "grpic_fields.cuh"
 
 using namespace grpic;
 typedef grpic_real real;
@@ -35,7 +36,7 @@ struct SortState {          // tile table of one species (keyed by the address o
 
 struct grpic_ctx {
   grpic_grid grid;
-  double a, r_min, r_max, small_angle, r0, h0, mass;
+  double a, r_min, r_max, small_angle, r0, h0, mass, k_J;
   int n_iter, tile_path, use_tma, early_exit;
   double last_dt;
   bool have_dt;
@@ -153,6 +154,19 @@ int check_current(grpic_ctx* ctx, const grpic_current* J, const SpeciesConst& sc
   return GRPIC_OK;
 }
 
+FieldGeom make_field_geom(const grpic_ctx* c) {
+  FieldGeom q;
+  q.n1 = c->grid.n1; q.n2 = c->grid.n2; q.ng = c->grid.nghost;
+  q.ld = c->grid.n2 + 2 * c->grid.nghost; q.rows = c->grid.n1 + 2 * c->grid.nghost;
+  q.r_lin = c->grid.r_map == 0 ? 1 : 0;
+  q.a = c->a; q.mass = c->mass; q.r_off = c->r0; q.h0 = c->h0;
+  q.log_rmin = q.r_lin ? 0.0 : std::log(c->r_min - c->r0);
+  q.dxi = q.r_lin ? 1.0 : std::log((c->r_max - c->r0) / (c->r_min - c->r0)) / c->grid.n1;
+  q.deta = M_PI / c->grid.n2;
+  q.r_min = c->r_min; q.dr = (c->r_max - c->r_min) / c->grid.n1;
+  return q;
+}
+
 inline bool general_map(const grpic_ctx* c) {
   return c->r0 != 0.0 || c->h0 != 0.0 || c->grid.r_map == 0 || c->mass != 1.0;
 }
@@ -214,6 +228,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->small_angle = 1e-5;                                  // SMALL_ANGLE_GR
   ctx->r0 = 0.0; ctx->h0 = 0.0;                             // A.3 map parameters
   ctx->mass = 1.0;                                          // r_g = M = 1
+  ctx->k_J = 4.0 * M_PI;                                    // coefficient of J in Ampere's law (Eq. 37)
   ctx->n_iter = 10;
   ctx->tile_path = 1;
   ctx->use_tma = 1;
@@ -285,6 +300,10 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
   if (!std::strcmp(key, "r0")) {
     if (!(v < ctx->r_min)) return fail(ctx, GRPIC_EINVAL, "r0 must be < r_min");
     ctx->r0 = v;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "k_J")) {
+    ctx->k_J = v;
     return GRPIC_OK;
   }
   if (!std::strcmp(key, "mass")) {
@@ -502,6 +521,57 @@ int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* stream) {
   CK(cudaMemcpyAsync(&h, ctx->d_counters + 4, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   CK(cudaStreamSynchronize((cudaStream_t)stream));
   *n_updates = (int64_t)h;
+  return GRPIC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Field-solver half: auxiliary fields, Faraday, Ampere
+// ------------------------------------------------------------------------------------------------
+int grpic_aux_fields(grpic_ctx* ctx, const grpic_fields* em, grpic_vec3* E, grpic_vec3* H, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!em || !em->D1 || !em->D2 || !em->D3 || !em->B1 || !em->B2 || !em->B3)
+    return fail(ctx, GRPIC_EINVAL, "a field component pointer is NULL");
+  if (!E && !H) return fail(ctx, GRPIC_EINVAL, "both outputs are NULL");
+  if ((E && (!E->F1 || !E->F2 || !E->F3)) || (H && (!H->F1 || !H->F2 || !H->F3)))
+    return fail(ctx, GRPIC_EINVAL, "an output component pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  FPtrs<real> F;
+  F.f[0] = em->D1; F.f[1] = em->D2; F.f[2] = em->D3; F.f[3] = em->B1; F.f[4] = em->B2; F.f[5] = em->B3;
+  V3<real> Ev{{E ? E->F1 : nullptr, E ? E->F2 : nullptr, E ? E->F3 : nullptr}};
+  V3<real> Hv{{H ? H->F1 : nullptr, H ? H->F2 : nullptr, H ? H->F3 : nullptr}};
+  const dim3 grid((q.n2 + 1 + 127) / 128, q.rows - 2);
+  k_aux_fields<real><<<grid, 128, 0, (cudaStream_t)stream>>>(q, F, Ev, Hv);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!B || !E || !B->F1 || !B->F2 || !B->F3 || !E->F1 || !E->F2 || !E->F3)
+    return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  if (q.rows < 5) return GRPIC_OK;
+  V3<real> Bv{{B->F1, B->F2, B->F3}};
+  CV3<real> Ev{{E->F1, E->F2, E->F3}};
+  const dim3 grid((q.n2 + 127) / 128, q.rows - 4);
+  k_faraday<real><<<grid, 128, 0, (cudaStream_t)stream>>>(q, Bv, Ev, dt);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic_current* J, double dt, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!D || !H || !D->F1 || !D->F2 || !D->F3 || !H->F1 || !H->F2 || !H->F3)
+    return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
+  if (J && (!J->J1 || !J->J2 || !J->J3)) return fail(ctx, GRPIC_EINVAL, "a current component pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  if (q.rows < 5) return GRPIC_OK;
+  V3<real> Dv{{D->F1, D->F2, D->F3}};
+  CV3<real> Hv{{H->F1, H->F2, H->F3}};
+  CV3<real> Jv{{J ? J->J1 : nullptr, J ? J->J2 : nullptr, J ? J->J3 : nullptr}};
+  const dim3 grid((q.n2 + 1 + 127) / 128, q.rows - 4);
+  k_ampere<real><<<grid, 128, 0, (cudaStream_t)stream>>>(q, Dv, Hv, Jv, ctx->k_J, dt);
+  CK(cudaGetLastError());
   return GRPIC_OK;
 }
 

@@ -21,7 +21,8 @@ GRPIC_OK, GRPIC_EINVAL, GRPIC_ENOMEM, GRPIC_ECUDA, GRPIC_ESTATE = 0, -1, -2, -3,
 
 EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int", "grpic_set_real",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
-           "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error"]
+           "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
+           "grpic_aux_fields", "grpic_faraday", "grpic_ampere"]
 
 
 class GrpicError(RuntimeError):
@@ -47,6 +48,10 @@ class _Particles(C.Structure):
 
 class _Fields(C.Structure):
     _fields_ = [(k, _vp) for k in ("D1", "D2", "D3", "B1", "B2", "B3")]
+
+
+class _Vec3(C.Structure):
+    _fields_ = [(k, _vp) for k in ("F1", "F2", "F3")]
 
 
 class _Current(C.Structure):
@@ -81,6 +86,9 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_updates_total.argtypes = [_vp, C.POINTER(C.c_int64), _vp]
     lib.grpic_step_host.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Fields), C.POINTER(_Current), C.c_double,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.grpic_aux_fields.argtypes = [_vp, C.POINTER(_Fields), C.POINTER(_Vec3), C.POINTER(_Vec3), _vp]
+    lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
+    lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
     want = 4 if precision == "f32" else 8
     if lib.grpic_real_bytes() != want:
         raise ImportError(f"{path} reports grpic_real of {lib.grpic_real_bytes()} bytes, expected {want}")
@@ -277,6 +285,27 @@ class Context:
         self._ck(self.lib.grpic_step_host(self.h, C.byref(ps), C.byref(fs) if fs else None,
                                           C.byref(js) if js else None, float(dt), C.byref(up), C.byref(down)))
         return int(up.value), int(down.value)
+
+    # ---- field-solver half (Sec. 3.3): dicts of torch CUDA tensors, keys as named ----
+    def aux_fields(self, fields, E=None, H=None, stream=None):
+        """E = dict(E1,E2,E3) and/or H = dict(H1,H2,H3) are written from fields = dict(D1..B3)."""
+        fs = _fields_struct(fields)
+        e = None if E is None else _Vec3(*[E[k].data_ptr() for k in ("E1", "E2", "E3")])
+        h = None if H is None else _Vec3(*[H[k].data_ptr() for k in ("H1", "H2", "H3")])
+        self._ck(self.lib.grpic_aux_fields(self.h, C.byref(fs), C.byref(e) if e else None, C.byref(h) if h else None,
+                                           _stream_ptr(stream)))
+
+    def faraday(self, B, E, dt, stream=None):
+        b = _Vec3(*[B[k].data_ptr() for k in ("B1", "B2", "B3")])
+        e = _Vec3(*[E[k].data_ptr() for k in ("E1", "E2", "E3")])
+        self._ck(self.lib.grpic_faraday(self.h, C.byref(b), C.byref(e), float(dt), _stream_ptr(stream)))
+
+    def ampere(self, D, H, J, dt, stream=None):
+        d = _Vec3(*[D[k].data_ptr() for k in ("D1", "D2", "D3")])
+        h = _Vec3(*[H[k].data_ptr() for k in ("H1", "H2", "H3")])
+        js = _current_struct(J)
+        self._ck(self.lib.grpic_ampere(self.h, C.byref(d), C.byref(h), C.byref(js) if js else None, float(dt),
+                                       _stream_ptr(stream)))
 
     def tile_size(self):
         return int(self.lib.grpic_tile_size())

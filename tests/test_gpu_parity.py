@@ -411,3 +411,78 @@ def test_early_exit_is_bit_identical_to_all_iterations(G, W, prec):
             assert np.array_equal(a[0][k], b[0][k]), k
     for k in a[1]:
         assert np.allclose(a[1][k], b[1][k], rtol=0, atol=TOL[prec]["J"] * np.abs(b[1][k]).max())
+
+
+# ------------------------------------------------------------------------------------------------
+# field-solver half: auxiliary fields, Faraday, Ampere against the oracle
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("kw", [dict(), dict(r0=0.5, h0=0.3), dict(linear_r=1), dict(linear_r=1, mass=0.0)])
+def test_field_solver_kernels(G, O, W, prec, kw):
+    """grpic_aux_fields / grpic_faraday / grpic_ampere element by element against the oracle on random fields and
+    currents (several thread blocks per row and a ragged tail in theta), on four maps; then div B and the Wald
+    stationarity are re-checked on the GPU output of the default map."""
+    import torch
+    mass = kw.get("mass", 1.0)
+    a = 0.9 if mass else 0.0
+    n1, n2, ng = 70, 150, 2
+    g = O.Grid(n1, n2, a, 1.3, 18.0, ng=ng, **kw)
+    ctx = G.Context(n1, n2, a, g.r_min, g.r_max, nghost=ng, precision=prec, r0=kw.get("r0"), h0=kw.get("h0"),
+                    r_map=0 if kw.get("linear_r") else 1, mass=kw.get("mass"))
+    rng = np.random.default_rng(11)
+    rt = np.float32 if prec == "f32" else np.float64
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    f = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in names}
+    J = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in ("J1", "J2", "J3")}
+    dev = lambda d: {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in d.items()}
+    tol = 2e-6 if prec == "f32" else 1e-12
+
+    def close(got, ref, what):
+        for k in ref:
+            r = ref[k]; x = got[k].cpu().numpy().astype(np.float64)
+            assert np.abs(x - r).max() <= tol * max(1.0, np.abs(r).max()), (what, k, np.abs(x - r).max(), np.abs(r).max())
+
+    fd = dev(f)
+    Ed = {k: torch.zeros(g.shape, dtype=G.torch_real(prec), device="cuda") for k in ("E1", "E2", "E3")}
+    Hd = {k: torch.zeros(g.shape, dtype=G.torch_real(prec), device="cuda") for k in ("H1", "H2", "H3")}
+    ctx.aux_fields(fd, Ed, Hd)
+    aux = O.aux_fields(g, f)
+    close({**Ed, **Hd}, aux, "aux")
+    # Faraday / Ampere from the oracle's aux fields rounded to the build's precision (same inputs on both sides)
+    auxr = {k: v.astype(rt).astype(np.float64) for k, v in aux.items()}
+    dt = 0.013
+    Bo = {k: f[k].copy() for k in ("B1", "B2", "B3")}; Do = {k: f[k].copy() for k in ("D1", "D2", "D3")}
+    O.faraday(g, Bo, auxr, dt); O.ampere(g, Do, auxr, J, dt)
+    Bd = {k: fd[k].clone() for k in ("B1", "B2", "B3")}; Dd = {k: fd[k].clone() for k in ("D1", "D2", "D3")}
+    ad = dev(auxr)
+    ctx.faraday(Bd, ad, dt); ctx.ampere(Dd, ad, dev(J), dt)
+    close(Bd, Bo, "faraday"); close(Dd, Do, "ampere")
+    # untouched entries: ghost columns beyond the axes and the outer two ghost rows
+    assert torch.equal(Bd["B1"][:2], fd["B1"][:2]) and torch.equal(Dd["D2"][:, :ng], fd["D2"][:, :ng])
+    assert torch.equal(Bd["B2"][:, ng], fd["B2"][:, ng])                  # B^2 on the axis is not evolved (P:449)
+    Dd2 = {k: fd[k].clone() for k in ("D1", "D2", "D3")}
+    ctx.ampere(Dd2, ad, None, dt)                                         # J = NULL: vacuum
+    Do2 = {k: f[k].copy() for k in ("D1", "D2", "D3")}
+    O.ampere(g, Do2, auxr, None, dt)
+    close(Dd2, Do2, "ampere vacuum")
+
+
+def test_field_solver_wald_stationary_on_gpu(G, O, W):
+    """The stationary Wald solution through the GPU kernels (FP64, 256x128, r >= 2.6): residual of one Faraday + Ampere
+    update below 1e-4 of the field everywhere, axis rows included (same bound as the oracle pin)."""
+    import torch
+    a = 0.9
+    dom = W.Domain(256, 128, a, 2.6, 20.0)
+    ctx = G.Context(dom.n1, dom.n2, a, dom.r_min, dom.r_max, nghost=dom.ng, precision="f64")
+    f = W.wald_fields(dom, 1.0)
+    fd = {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in f.items()}
+    E = {k: torch.zeros(dom.shape, dtype=torch.float64, device="cuda") for k in ("E1", "E2", "E3")}
+    H = {k: torch.zeros(dom.shape, dtype=torch.float64, device="cuda") for k in ("H1", "H2", "H3")}
+    ctx.aux_fields(fd, E, H)
+    B = {k: fd[k].clone() for k in ("B1", "B2", "B3")}; D = {k: fd[k].clone() for k in ("D1", "D2", "D3")}
+    ctx.faraday(B, E, 1.0); ctx.ampere(D, H, None, 1.0)
+    G_ = dom.ng
+    sl = (slice(G_ + 2, G_ + dom.n1 - 2), slice(G_, G_ + dom.n2 + 1))
+    for k, new in list(B.items()) + list(D.items()):
+        r = float((new - fd[k])[sl].abs().max() / fd[k][sl].abs().max())
+        assert r < 1e-4, (k, r)
