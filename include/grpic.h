@@ -175,6 +175,21 @@ int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt,
  * form Eq. 45 with the polar area of App. A. */
 int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic_current* J, double dt, void* cuda_stream);
 
+/* Field side of one PIC timestep (Sec. 3.4), built from the three operations above.  The state holds
+ * (n-3/2)B, (n-1/2)B, (n-1)D, (n)D; all arrays caller-owned device memory; library scratch: 12 grid arrays.
+ *   grpic_fields_prepare  step 2, Eq. 46-48: B_n <- (n)B, the magnetic field aligned in time with (n)D for the push
+ *                         (grpic_interp_push / grpic_step then take D = state.D, B = B_n).
+ *   grpic_fields_advance  steps 5-7, Eq. 51-56, after the deposit of (n+1/2)J: (n)J = ((n-1/2)J + (n+1/2)J)/2;
+ *                         (n)E,(n)H; main Faraday (n-1/2)B -> (n+1/2)B; auxiliary Ampere (n-1/2)D -> (n+1/2)D with
+ *                         (n)H,(n)J; (n+1/2)H; final Ampere (n)D -> (n+1)D with (n+1/2)H,(n+1/2)J.
+ *                         On return the state holds (n-1/2)B, (n+1/2)B, (n)D, (n+1)D in B_prev, B, D_prev, D.
+ *                         J_prev = (n-1/2)J and J = (n+1/2)J, or both NULL (vacuum).
+ * Errors: EINVAL, ENOMEM (scratch), ECUDA. */
+typedef struct { grpic_vec3 B_prev, B, D_prev, D; } grpic_field_state;
+int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3* B_n, double dt, void* cuda_stream);
+int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3* B_n, const grpic_current* J_prev,
+                         const grpic_current* J, double dt, void* cuda_stream);
+
 /* End-to-end convenience: every pointer in p, fields and J is HOST memory (pinned or pageable).
  * Copies fields and particle columns to library-owned device buffers in chunks, runs the fused step
  * chunk by chunk (copies overlapped with compute on two streams), accumulates J on the device and

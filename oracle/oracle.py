@@ -330,3 +330,37 @@ def sort_reference(g: Grid, p: Particles, tile: int):
         if isinstance(v, np.ndarray):
             setattr(q, k, v[perm].copy())
     return q, perm, key[perm]
+
+
+# ----------------------------------------------------------------------------------------------
+# Field side of one PIC timestep (Sec. 3.4), plain numpy around the three operations above.
+# state = dict(B_prev = (n-3/2)B, B = (n-1/2)B, D_prev = (n-1)D, D = (n)D), each a dict of three float64 arrays.
+# ----------------------------------------------------------------------------------------------
+def _avg(x, y, keys):
+    return {k: 0.5 * (x[k] + y[k]) for k in keys}
+
+
+def fields_prepare(g: Grid, state: dict, dt: float) -> dict:
+    """Step 2 (Eq. 46-48): returns (n)B, the magnetic field aligned with (n)D for the particle push."""
+    kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+    B_nm1 = _avg(state["B_prev"], state["B"], kb)                       # (n-1)B
+    D_half = _avg(state["D_prev"], state["D"], kd)                      # (n-1/2)D
+    E_half = aux_fields(g, {**state["B"], **D_half})                    # (n-1/2)E from (n-1/2)B, (n-1/2)D
+    B_n = {k: np.array(v) for k, v in B_nm1.items()}
+    faraday(g, B_n, E_half, dt)                                         # (n-1)B -> (n)B
+    return B_n
+
+
+def fields_advance(g: Grid, state: dict, B_n: dict, J_prev, J, dt: float, kJ: float = 4.0 * np.pi) -> dict:
+    """Steps 5-7 (Eq. 51-56): state at (n+1); J_prev = (n-1/2)J, J = (n+1/2)J (dicts or None for vacuum)."""
+    kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+    J_n = None if J is None else _avg(J_prev, J, ("J1", "J2", "J3"))    # Eq. 51
+    aux_n = aux_fields(g, {**B_n, **state["D"]})                        # Eq. 52
+    B_new = {k: np.array(v) for k, v in state["B"].items()}
+    faraday(g, B_new, aux_n, dt)                                        # Eq. 53: (n-1/2)B -> (n+1/2)B
+    D_half = _avg(state["D_prev"], state["D"], kd)                      # (n-1/2)D
+    ampere(g, D_half, aux_n, J_n, dt, kJ)                               # Eq. 54: -> (n+1/2)D
+    aux_h = aux_fields(g, {**B_new, **D_half})                          # Eq. 55
+    D_new = {k: np.array(v) for k, v in state["D"].items()}
+    ampere(g, D_new, aux_h, J, dt, kJ)                                  # Eq. 56: (n)D -> (n+1)D
+    return dict(B_prev=state["B"], B=B_new, D_prev=state["D"], D=D_new)

@@ -57,6 +57,8 @@ struct grpic_ctx {
   void* h_fields;
   size_t h_fields_bytes;
   cudaStream_t h_streams[3];
+  real* f_scratch;          // 12 grid arrays for the field side of the PIC loop: E[3] H[3] Dh[3] Jn[3]
+  size_t f_scratch_cells;
   bool h_streams_ok;
 };
 
@@ -239,6 +241,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->cap_particles = 0;
   ctx->d_scratch = nullptr; ctx->scratch_bytes = 0;
   for (auto& q : ctx->h_dev) q = nullptr;
+  ctx->f_scratch = nullptr; ctx->f_scratch_cells = 0;
   ctx->h_cap = 0; ctx->h_fields = nullptr; ctx->h_fields_bytes = 0; ctx->h_streams_ok = false;
   cudaGetDevice(&ctx->device);
   e = cudaMalloc(&ctx->d_counters, 8 * sizeof(unsigned long long));
@@ -263,6 +266,7 @@ int grpic_destroy(grpic_ctx* ctx) {
   cudaFree(ctx->d_scratch);
   for (auto q : ctx->h_dev) cudaFree(q);
   cudaFree(ctx->h_fields);
+  cudaFree(ctx->f_scratch);
   if (ctx->h_streams_ok) for (auto& q : ctx->h_streams) cudaStreamDestroy(q);
   delete ctx;
   return GRPIC_OK;
@@ -571,6 +575,108 @@ int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic
   CV3<real> Jv{{J ? J->J1 : nullptr, J ? J->J2 : nullptr, J ? J->J3 : nullptr}};
   const dim3 grid((q.n2 + 1 + 127) / 128, q.rows - 4);
   k_ampere<real><<<grid, 128, 0, (cudaStream_t)stream>>>(q, Dv, Hv, Jv, ctx->k_J, dt);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+// ---- field side of one PIC timestep (Sec. 3.4) ----
+namespace {
+int field_scratch(grpic_ctx* ctx, size_t cells) {
+  if (ctx->f_scratch_cells >= cells) return GRPIC_OK;
+  cudaFree(ctx->f_scratch); ctx->f_scratch = nullptr; ctx->f_scratch_cells = 0;
+  if (cudaMalloc((void**)&ctx->f_scratch, 12 * cells * sizeof(real)) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(ctx, GRPIC_ENOMEM, "field scratch allocation failed");
+  }
+  ctx->f_scratch_cells = cells;
+  return GRPIC_OK;
+}
+bool vec3_ok(const grpic_vec3* v) { return v && v->F1 && v->F2 && v->F3; }
+void average3(real* out, const real* a1, const real* a2, const real* a3, const real* b1, const real* b2, const real* b3,
+              size_t cells, cudaStream_t st) {
+  const unsigned nb = (unsigned)((cells + 255) / 256);
+  k_average<real><<<nb, 256, 0, st>>>(out, a1, b1, (int64_t)cells);
+  k_average<real><<<nb, 256, 0, st>>>(out + cells, a2, b2, (int64_t)cells);
+  k_average<real><<<nb, 256, 0, st>>>(out + 2 * cells, a3, b3, (int64_t)cells);
+}
+}  // namespace
+
+int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3* B_n, double dt, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!s || !vec3_ok(&s->B_prev) || !vec3_ok(&s->B) || !vec3_ok(&s->D_prev) || !vec3_ok(&s->D) || !vec3_ok(B_n))
+    return fail(ctx, GRPIC_EINVAL, "a field pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  const size_t cells = (size_t)q.rows * q.ld;
+  int rc = field_scratch(ctx, cells);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  real* E = ctx->f_scratch; real* Dh = ctx->f_scratch + 6 * cells;
+  const unsigned nb = (unsigned)((cells + 255) / 256);
+  // Eq. 46: (n-1)B = ((n-3/2)B + (n-1/2)B)/2 -> B_n;  (n-1/2)D = ((n-1)D + (n)D)/2
+  k_average<real><<<nb, 256, 0, st>>>(B_n->F1, s->B_prev.F1, s->B.F1, (int64_t)cells);
+  k_average<real><<<nb, 256, 0, st>>>(B_n->F2, s->B_prev.F2, s->B.F2, (int64_t)cells);
+  k_average<real><<<nb, 256, 0, st>>>(B_n->F3, s->B_prev.F3, s->B.F3, (int64_t)cells);
+  average3(Dh, s->D_prev.F1, s->D_prev.F2, s->D_prev.F3, s->D.F1, s->D.F2, s->D.F3, cells, st);
+  // Eq. 47: (n-1/2)E from (n-1/2)B, (n-1/2)D
+  FPtrs<real> F;
+  F.f[0] = Dh; F.f[1] = Dh + cells; F.f[2] = Dh + 2 * cells; F.f[3] = s->B.F1; F.f[4] = s->B.F2; F.f[5] = s->B.F3;
+  V3<real> Ev{{E, E + cells, E + 2 * cells}}, none{{nullptr, nullptr, nullptr}};
+  k_aux_fields<real><<<dim3((q.n2 + 1 + 127) / 128, q.rows - 2), 128, 0, st>>>(q, F, Ev, none);
+  // Eq. 48: (n-1)B -> (n)B
+  if (q.rows >= 5) {
+    V3<real> Bv{{B_n->F1, B_n->F2, B_n->F3}};
+    CV3<real> Ec{{E, E + cells, E + 2 * cells}};
+    k_faraday<real><<<dim3((q.n2 + 127) / 128, q.rows - 4), 128, 0, st>>>(q, Bv, Ec, dt);
+  }
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
+int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3* B_n, const grpic_current* J_prev,
+                         const grpic_current* J, double dt, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!s || !vec3_ok(&s->B_prev) || !vec3_ok(&s->B) || !vec3_ok(&s->D_prev) || !vec3_ok(&s->D) || !vec3_ok(B_n))
+    return fail(ctx, GRPIC_EINVAL, "a field pointer is NULL");
+  if ((J == nullptr) != (J_prev == nullptr)) return fail(ctx, GRPIC_EINVAL, "J and J_prev must both be given or both be NULL");
+  if (J && (!J->J1 || !J->J2 || !J->J3 || !J_prev->J1 || !J_prev->J2 || !J_prev->J3))
+    return fail(ctx, GRPIC_EINVAL, "a current component pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  const size_t cells = (size_t)q.rows * q.ld, bytes = cells * sizeof(real);
+  int rc = field_scratch(ctx, cells);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  real *E = ctx->f_scratch, *H = E + 3 * cells, *Dh = E + 6 * cells, *Jn = E + 9 * cells;
+  const dim3 g_aux((q.n2 + 1 + 127) / 128, q.rows - 2), g_far((q.n2 + 127) / 128, q.rows - 4), g_amp((q.n2 + 1 + 127) / 128, q.rows - 4);
+  V3<real> Ev{{E, E + cells, E + 2 * cells}}, Hv{{H, H + cells, H + 2 * cells}}, none{{nullptr, nullptr, nullptr}};
+  CV3<real> Ec{{E, E + cells, E + 2 * cells}}, Hc{{H, H + cells, H + 2 * cells}};
+  // Eq. 51: (n)J = ((n-1/2)J + (n+1/2)J)/2
+  CV3<real> Jnc{{nullptr, nullptr, nullptr}}, Jc{{nullptr, nullptr, nullptr}};
+  if (J) {
+    average3(Jn, J_prev->J1, J_prev->J2, J_prev->J3, J->J1, J->J2, J->J3, cells, st);
+    Jnc = CV3<real>{{Jn, Jn + cells, Jn + 2 * cells}};
+    Jc = CV3<real>{{J->J1, J->J2, J->J3}};
+  }
+  // Eq. 52: (n)E, (n)H from (n)B, (n)D
+  FPtrs<real> F;
+  F.f[0] = s->D.F1; F.f[1] = s->D.F2; F.f[2] = s->D.F3; F.f[3] = B_n->F1; F.f[4] = B_n->F2; F.f[5] = B_n->F3;
+  k_aux_fields<real><<<g_aux, 128, 0, st>>>(q, F, Ev, Hv);
+  // (n-1/2)D before D is touched
+  average3(Dh, s->D_prev.F1, s->D_prev.F2, s->D_prev.F3, s->D.F1, s->D.F2, s->D.F3, cells, st);
+  // Eq. 53: (n-1/2)B -> (n+1/2)B; the old (n-1/2)B moves to B_prev
+  CK(cudaMemcpyAsync(s->B_prev.F1, s->B.F1, bytes, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(s->B_prev.F2, s->B.F2, bytes, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(s->B_prev.F3, s->B.F3, bytes, cudaMemcpyDeviceToDevice, st));
+  if (q.rows >= 5) k_faraday<real><<<g_far, 128, 0, st>>>(q, V3<real>{{s->B.F1, s->B.F2, s->B.F3}}, Ec, dt);
+  // Eq. 54: (n-1/2)D -> (n+1/2)D with (n)H, (n)J
+  if (q.rows >= 5) k_ampere<real><<<g_amp, 128, 0, st>>>(q, V3<real>{{Dh, Dh + cells, Dh + 2 * cells}}, Hc, Jnc, ctx->k_J, dt);
+  // Eq. 55: (n+1/2)H from (n+1/2)B, (n+1/2)D
+  F.f[0] = Dh; F.f[1] = Dh + cells; F.f[2] = Dh + 2 * cells; F.f[3] = s->B.F1; F.f[4] = s->B.F2; F.f[5] = s->B.F3;
+  k_aux_fields<real><<<g_aux, 128, 0, st>>>(q, F, none, Hv);
+  // Eq. 56: (n)D -> (n+1)D with (n+1/2)H, (n+1/2)J; the old (n)D moves to D_prev
+  CK(cudaMemcpyAsync(s->D_prev.F1, s->D.F1, bytes, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(s->D_prev.F2, s->D.F2, bytes, cudaMemcpyDeviceToDevice, st));
+  CK(cudaMemcpyAsync(s->D_prev.F3, s->D.F3, bytes, cudaMemcpyDeviceToDevice, st));
+  if (q.rows >= 5) k_ampere<real><<<g_amp, 128, 0, st>>>(q, V3<real>{{s->D.F1, s->D.F2, s->D.F3}}, Hc, Jc, ctx->k_J, dt);
   CK(cudaGetLastError());
   return GRPIC_OK;
 }

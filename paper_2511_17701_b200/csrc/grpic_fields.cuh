@@ -174,4 +174,11 @@ __global__ void __launch_bounds__(128) k_ampere(const FieldGeom q, const V3<T> D
   }
 }
 
+// out = (a + b)/2 over whole arrays (the time averages of Eq. 46 and Eq. 51)
+template <typename T>
+__global__ void __launch_bounds__(256) k_average(T* out, const T* a, const T* b, int64_t n) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) out[k] = T(0.5) * (a[k] + b[k]);
+}
+
 }  // namespace grpic

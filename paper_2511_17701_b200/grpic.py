@@ -22,7 +22,7 @@ GRPIC_OK, GRPIC_EINVAL, GRPIC_ENOMEM, GRPIC_ECUDA, GRPIC_ESTATE = 0, -1, -2, -3,
 EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int", "grpic_set_real",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
-           "grpic_aux_fields", "grpic_faraday", "grpic_ampere"]
+           "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance"]
 
 
 class GrpicError(RuntimeError):
@@ -52,6 +52,10 @@ class _Fields(C.Structure):
 
 class _Vec3(C.Structure):
     _fields_ = [(k, _vp) for k in ("F1", "F2", "F3")]
+
+
+class _FieldState(C.Structure):
+    _fields_ = [("B_prev", _Vec3), ("B", _Vec3), ("D_prev", _Vec3), ("D", _Vec3)]
 
 
 class _Current(C.Structure):
@@ -89,6 +93,9 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_aux_fields.argtypes = [_vp, C.POINTER(_Fields), C.POINTER(_Vec3), C.POINTER(_Vec3), _vp]
     lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
+    lib.grpic_fields_prepare.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.c_double, _vp]
+    lib.grpic_fields_advance.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.POINTER(_Current),
+                                         C.POINTER(_Current), C.c_double, _vp]
     want = 4 if precision == "f32" else 8
     if lib.grpic_real_bytes() != want:
         raise ImportError(f"{path} reports grpic_real of {lib.grpic_real_bytes()} bytes, expected {want}")
@@ -306,6 +313,26 @@ class Context:
         js = _current_struct(J)
         self._ck(self.lib.grpic_ampere(self.h, C.byref(d), C.byref(h), C.byref(js) if js else None, float(dt),
                                        _stream_ptr(stream)))
+
+    @staticmethod
+    def _state_struct(state):
+        v = lambda d, ks: _Vec3(*[d[k].data_ptr() for k in ks])
+        kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+        return _FieldState(v(state["B_prev"], kb), v(state["B"], kb), v(state["D_prev"], kd), v(state["D"], kd))
+
+    def fields_prepare(self, state, B_n, dt, stream=None):
+        """state = dict(B_prev, B, D_prev, D) of dicts of tensors; B_n = dict(B1,B2,B3) receives (n)B (Eq. 46-48)."""
+        ss = self._state_struct(state)
+        bn = _Vec3(*[B_n[k].data_ptr() for k in ("B1", "B2", "B3")])
+        self._ck(self.lib.grpic_fields_prepare(self.h, C.byref(ss), C.byref(bn), float(dt), _stream_ptr(stream)))
+
+    def fields_advance(self, state, B_n, J_prev, J, dt, stream=None):
+        """Eq. 51-56; the tensors of `state` are updated in place to (n-1/2)B, (n+1/2)B, (n)D, (n+1)D."""
+        ss = self._state_struct(state)
+        bn = _Vec3(*[B_n[k].data_ptr() for k in ("B1", "B2", "B3")])
+        jp, jn = _current_struct(J_prev), _current_struct(J)
+        self._ck(self.lib.grpic_fields_advance(self.h, C.byref(ss), C.byref(bn), C.byref(jp) if jp else None,
+                                               C.byref(jn) if jn else None, float(dt), _stream_ptr(stream)))
 
     def tile_size(self):
         return int(self.lib.grpic_tile_size())

@@ -486,3 +486,52 @@ def test_field_solver_wald_stationary_on_gpu(G, O, W):
     for k, new in list(B.items()) + list(D.items()):
         r = float((new - fd[k])[sl].abs().max() / fd[k][sl].abs().max())
         assert r < 1e-4, (k, r)
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_full_pic_cycle_against_the_oracle(G, O, W, prec):
+    """Four complete timesteps of Sec. 3.4 on the GPU and in the oracle, each side with its own state:
+    fields_prepare (Eq. 46-48) -> push with (n)B, (n)D -> deposit (n+1/2)J -> fields_advance (Eq. 51-56).
+    Tiny magnetosphere (config 1 shape, Wald field, e+- pairs); tolerances as for the per-step parity but accumulated
+    over the four steps (x2 per step for f32)."""
+    import torch
+    wl = W.config_tiny(shrink=2)
+    dom = wl.dom
+    g = grid_from_domain(O, dom)
+    ctx = _ctx(G, dom, prec)
+    rt = np.float32 if prec == "f32" else np.float64
+    kb, kd, kj = ("B1", "B2", "B3"), ("D1", "D2", "D3"), ("J1", "J2", "J3")
+    f = {k: np.asarray(v, rt).astype(np.float64) for k, v in wl.fields.items()}
+    cp = lambda ks: {k: f[k].copy() for k in ks}
+    so = dict(B_prev=cp(kb), B=cp(kb), D_prev=cp(kd), D=cp(kd))
+    td = lambda d: {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in d.items()}
+    sg = {k: td(v) for k, v in so.items()}
+    zeros = lambda ks: {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ks}
+    Bn_g = zeros(kb)
+    sets = [G.ParticleSet.from_host(sp, prec) for sp in wl.species]
+    ops = [oracle_from_cols(O, ps.to_numpy(), ps.q_over_m, ps.charge, ps.massive) for ps in sets]
+    Jprev_g, Jprev_o = zeros(kj), {k: np.zeros(g.shape) for k in kj}
+    dt = wl.dt
+    for step in range(4):
+        ctx.fields_prepare(sg, Bn_g, dt)
+        Bn_o = O.fields_prepare(g, so, dt)
+        Jg, Jo = zeros(kj), {k: np.zeros(g.shape) for k in kj}
+        for ps, op in zip(sets, ops):
+            ctx.step(ps, {**sg["D"], **Bn_g}, Jg, dt)
+            O.push(g, op, {**so["D"], **Bn_o}, dt)
+            O.deposit(g, op, dt, Jo)
+        ctx.fields_advance(sg, Bn_g, Jprev_g, Jg, dt)
+        so = O.fields_advance(g, so, Bn_o, Jprev_o, Jo, dt)
+        Jprev_g, Jprev_o = Jg, Jo
+    tol = (1e-4 if prec == "f32" else 1e-10)
+    for name in ("B_prev", "B", "D_prev", "D"):
+        for k, ref in so[name].items():
+            got = sg[name][k].cpu().numpy().astype(np.float64)
+            err = np.abs(got - ref).max() / max(1e-300, np.abs(ref).max())
+            assert err < tol, (name, k, err)
+    for ps, op in zip(sets, ops):
+        c = ps.to_numpy()
+        same = (c["i1"] == op.i1) & (c["i2"] == op.i2) & (c["tag"] == op.tag)
+        assert same.mean() > (0.999 if prec == "f32" else 1.0 - 1e-9)
+        ex = np.abs((c["i1"] + c["dx1"].astype(np.float64)) - (op.i1 + op.dx1))[c["tag"] != 0].max()
+        assert ex < (1e-4 if prec == "f32" else 1e-10), ex

@@ -133,3 +133,38 @@ def test_flat_limit_of_the_auxiliary_fields(O):
     assert np.allclose(aux["H1"][sl], (dr ** 2 * f["B1"])[sl], rtol=1e-13)
     assert np.allclose(aux["H2"][sl], ((dth * r(0.5)) ** 2 * f["B2"])[sl], rtol=1e-13)
     assert np.allclose(aux["H3"][sl], ((r(0.5) * np.sin(th(0.5))) ** 2 * f["B3"])[sl], rtol=1e-12)
+
+
+def _wald_state(W, dom):
+    f = W.wald_fields(dom, 1.0)
+    cp = lambda ks: {k: np.array(f[k]) for k in ks}
+    kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+    return f, dict(B_prev=cp(kb), B=cp(kb), D_prev=cp(kd), D=cp(kd))
+
+
+def test_pic_loop_keeps_the_wald_vacuum_stationary(O, W):
+    """Field side of the PIC loop (Sec. 3.4, Eq. 46-56) in vacuum, started from the analytic Wald solution with the
+    radial ghost rows held at it (paper's Sec. 4.2 test, at small size): the solution stays within a
+    bounded distance of the analytic one (no growth between t = 3 and t = 12), that distance shrinks with the cell
+    size, and the time-aligned (n)B of step 2 differs from the stationary B by O(dt * residual) only."""
+    a = 0.9
+    err = {}
+    for n in (32, 64):
+        dom = W.Domain(n, n // 2, a, 0.9 * W.horizon_radius(a), 20.0)
+        g = O.Grid(dom.n1, dom.n2, a, dom.r_min, dom.r_max)
+        f, st = _wald_state(W, dom)
+        dt = 0.5 * W.cfl_dt(dom) * (n / 32)                              # same physical dt on both grids
+        G = dom.ng
+        sl = (slice(G, G + dom.n1), slice(G, G + dom.n2 + 1))
+        rel = lambda d: max(np.abs((d[k] - f[k])[sl]).max() / np.abs(f[k][sl]).max() for k in d)
+        steps = int(round(12.0 / dt))
+        for step in range(1, steps + 1):
+            Bn = O.fields_prepare(g, st, dt)
+            if step == 1:
+                assert rel(Bn) < 5e-3
+            st = O.fields_advance(g, st, Bn, None, None, dt)
+            if step == steps // 4:
+                err[(n, "early")] = max(rel(st["B"]), rel(st["D"]))
+        err[(n, "late")] = max(rel(st["B"]), rel(st["D"]))
+    assert err[(32, "late")] < 2.0 * err[(32, "early")] and err[(64, "late")] < 2.0 * err[(64, "early")], err   # bounded
+    assert err[(32, "late")] < 0.1 and err[(64, "late")] < 0.6 * err[(32, "late")], err                           # converging
