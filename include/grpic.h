@@ -175,6 +175,13 @@ int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt,
  * form Eq. 45 with the polar area of App. A. */
 int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic_current* J, double dt, void* cuda_stream);
 
+/* Field boundary conditions (Sec. 3.3.3), in place on D^i and B^i: the ghost columns beyond the two polar
+ * axes by reflection (r- and phi-components even, theta-components odd; Fig. 1), B^2 = D^3 = 0 on the axes, and,
+ * if n_const >= 0, the constant layer inside the horizon: rows i1 in [-nghost, n_const] take the values of row
+ * n_const + 1 (n_const = number of current-filter passes).  The absorbing MATCH layer at the outer edge
+ * (paper I) is not part of this call.  Errors: EINVAL, ECUDA. */
+int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const, void* cuda_stream);
+
 /* Field side of one PIC timestep (Sec. 3.4), built from the three operations above.  The state holds
  * (n-3/2)B, (n-1/2)B, (n-1)D, (n)D; all arrays caller-owned device memory; library scratch: 12 grid arrays.
  *   grpic_fields_prepare  step 2, Eq. 46-48: B_n <- (n)B, the magnetic field aligned in time with (n)D for the push

@@ -364,3 +364,35 @@ def fields_advance(g: Grid, state: dict, B_n: dict, J_prev, J, dt: float, kJ: fl
     D_new = {k: np.array(v) for k, v in state["D"].items()}
     ampere(g, D_new, aux_h, J, dt, kJ)                                  # Eq. 56: (n)D -> (n+1)D
     return dict(B_prev=state["B"], B=B_new, D_prev=state["D"], D=D_new)
+
+
+# ----------------------------------------------------------------------------------------------
+# Field boundary conditions (Sec. 3.3.3; reading R-F4 of DESIGN.md): reflection across the polar axes of the
+# ghost columns, zero for the components that vanish on the axes, constant layer inside the horizon.
+# Parity of the contravariant code-basis components under theta -> -theta: r-components even, theta-components odd
+# (Fig. 1); phi-components even (not stated; what the analytic continuation of an axisymmetric field gives).
+# ----------------------------------------------------------------------------------------------
+_AXIS_PARITY = {"D1": (+1, 0.0), "D2": (-1, 0.5), "D3": (+1, 0.0), "B1": (+1, 0.5), "B2": (-1, 0.0), "B3": (+1, 0.5)}
+
+
+def field_bc(g: Grid, fields: dict, n_const: int = -1) -> dict:
+    """In place on dict(D1..B3) of float64 arrays; n_const >= 0: rows i1 in [-ng, n_const] take the values of row
+    n_const + 1 (n_const = number of current-filter passes n_f)."""
+    G, n2 = g.ng, g.n2
+    for k, (par, off) in _AXIS_PARITY.items():
+        A = fields[k]
+        for m in range(1, G + 1):
+            if off == 0.0:                       # samples at integer j: ghost j = -m mirrors j = +m; j = n2+m mirrors n2-m
+                A[:, G - m] = par * A[:, G + m]
+                if G + n2 + m < A.shape[1]:
+                    A[:, G + n2 + m] = par * A[:, G + n2 - m]
+            else:                                # samples at j+1/2: ghost j = -m (+1/2) mirrors j = m-1 (+1/2)
+                A[:, G - m] = par * A[:, G + m - 1]
+                A[:, G + n2 + m - 1] = par * A[:, G + n2 - m]
+    for k in ("B2", "D3"):                       # vanish on the axes by symmetry (P:395, P:449)
+        fields[k][:, G] = 0.0
+        fields[k][:, G + n2] = 0.0
+    if n_const >= 0:
+        for A in fields.values():
+            A[: G + n_const + 1, :] = A[G + n_const + 1, :]
+    return fields

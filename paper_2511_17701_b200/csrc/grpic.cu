@@ -579,6 +579,22 @@ int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic
   return GRPIC_OK;
 }
 
+int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!D || !B || !D->F1 || !D->F2 || !D->F3 || !B->F1 || !B->F2 || !B->F3)
+    return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
+  const FieldGeom q = make_field_geom(ctx);
+  if (n_const >= q.n1) return fail(ctx, GRPIC_EINVAL, "n_const must be < n1");
+  if (q.n2 < q.ng) return fail(ctx, GRPIC_EINVAL, "n2 must be >= nghost for the axis reflection");
+  V3<real> Dv{{D->F1, D->F2, D->F3}}, Bv{{B->F1, B->F2, B->F3}};
+  cudaStream_t st = (cudaStream_t)stream;
+  k_field_bc_axis<real><<<dim3(1, q.rows, 6), 128, 0, st>>>(q, Dv, Bv);
+  if (n_const >= 0)
+    k_field_bc_layer<real><<<dim3((q.ld + 127) / 128, q.ng + n_const + 1, 6), 128, 0, st>>>(q, Dv, Bv, n_const);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
 // ---- field side of one PIC timestep (Sec. 3.4) ----
 namespace {
 int field_scratch(grpic_ctx* ctx, size_t cells) {

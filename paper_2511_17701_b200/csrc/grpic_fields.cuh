@@ -174,6 +174,39 @@ __global__ void __launch_bounds__(128) k_ampere(const FieldGeom q, const V3<T> D
   }
 }
 
+// Field boundary conditions (Sec. 3.3.3; R-F4): ghost columns beyond the polar axes by reflection
+// (r- and phi-components even, theta-components odd), B^2 = D^3 = 0 on the axes, then the constant layer inside the
+// horizon: rows i1 in [-ng, n_const] take the values of row n_const + 1.  One thread per (row, column); component
+// c = blockIdx.z in the order D1 D2 D3 B1 B2 B3.
+template <typename T>
+__global__ void __launch_bounds__(128) k_field_bc_axis(const FieldGeom q, const V3<T> D, const V3<T> B) {
+  const int c = blockIdx.z, a1 = blockIdx.y, t = threadIdx.x + blockIdx.x * blockDim.x;
+  if (t >= 2 * q.ng + 2) return;
+  T* A = c < 3 ? D.f[c] : B.f[c - 3];
+  const bool half = (c == 1 || c == 3 || c == 5);            // sampled at j + 1/2
+  const T par = (c == 1 || c == 4) ? T(-1) : T(1);           // theta-components are odd
+  T* row = A + (int64_t)a1 * q.ld;
+  const int G = q.ng, n2 = q.n2;
+  if (t < q.ng) {                                            // ghosts below theta = 0: m = t + 1
+    const int m = t + 1;
+    row[G - m] = par * row[half ? G + m - 1 : G + m];
+  } else if (t < 2 * q.ng) {                                 // ghosts beyond theta = pi
+    const int m = t - q.ng + 1;
+    const int dst = half ? G + n2 + m - 1 : G + n2 + m;
+    if (dst < q.ld) row[dst] = par * row[G + n2 - m];
+  } else if (c == 2 || c == 4) {                             // D3, B2 on the axes
+    row[t == 2 * q.ng ? G : G + n2] = T(0);
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_field_bc_layer(const FieldGeom q, const V3<T> D, const V3<T> B, int n_const) {
+  const int c = blockIdx.z, a1 = blockIdx.y, a2 = threadIdx.x + blockIdx.x * blockDim.x;
+  if (a2 >= q.ld || a1 > q.ng + n_const) return;
+  T* A = c < 3 ? D.f[c] : B.f[c - 3];
+  A[(int64_t)a1 * q.ld + a2] = A[(int64_t)(q.ng + n_const + 1) * q.ld + a2];
+}
+
 // out = (a + b)/2 over whole arrays (the time averages of Eq. 46 and Eq. 51)
 template <typename T>
 __global__ void __launch_bounds__(256) k_average(T* out, const T* a, const T* b, int64_t n) {

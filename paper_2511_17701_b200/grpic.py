@@ -22,7 +22,8 @@ GRPIC_OK, GRPIC_EINVAL, GRPIC_ENOMEM, GRPIC_ECUDA, GRPIC_ESTATE = 0, -1, -2, -3,
 EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int", "grpic_set_real",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
-           "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance"]
+           "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
+           "grpic_field_bc"]
 
 
 class GrpicError(RuntimeError):
@@ -93,6 +94,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_aux_fields.argtypes = [_vp, C.POINTER(_Fields), C.POINTER(_Vec3), C.POINTER(_Vec3), _vp]
     lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
+    lib.grpic_field_bc.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_int32, _vp]
     lib.grpic_fields_prepare.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_fields_advance.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.POINTER(_Current),
                                          C.POINTER(_Current), C.c_double, _vp]
@@ -313,6 +315,12 @@ class Context:
         js = _current_struct(J)
         self._ck(self.lib.grpic_ampere(self.h, C.byref(d), C.byref(h), C.byref(js) if js else None, float(dt),
                                        _stream_ptr(stream)))
+
+    def field_bc(self, fields, n_const=-1, stream=None):
+        """Axis reflection of the ghost columns, zeros on the axes, constant layer inside the horizon (in place)."""
+        d = _Vec3(*[fields[k].data_ptr() for k in ("D1", "D2", "D3")])
+        b = _Vec3(*[fields[k].data_ptr() for k in ("B1", "B2", "B3")])
+        self._ck(self.lib.grpic_field_bc(self.h, C.byref(d), C.byref(b), int(n_const), _stream_ptr(stream)))
 
     @staticmethod
     def _state_struct(state):

@@ -535,3 +535,21 @@ def test_full_pic_cycle_against_the_oracle(G, O, W, prec):
         assert same.mean() > (0.999 if prec == "f32" else 1.0 - 1e-9)
         ex = np.abs((c["i1"] + c["dx1"].astype(np.float64)) - (op.i1 + op.dx1))[c["tag"] != 0].max()
         assert ex < (1e-4 if prec == "f32" else 1e-10), ex
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("ng", [1, 2, 3])
+def test_field_bc(G, O, W, prec, ng):
+    """grpic_field_bc against the oracle on random arrays: bit-exact (copies and sign flips only)."""
+    import torch
+    g = O.Grid(20, 150, 0.9, 1.3, 15.0, ng=ng)
+    ctx = G.Context(g.n1, g.n2, 0.9, g.r_min, g.r_max, nghost=ng, precision=prec)
+    rng = np.random.default_rng(ng)
+    rt = np.float32 if prec == "f32" else np.float64
+    f = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in ("D1", "D2", "D3", "B1", "B2", "B3")}
+    for n_const in (-1, 0, 3):
+        fd = {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in f.items()}
+        ctx.field_bc(fd, n_const)
+        ref = O.field_bc(g, {k: v.copy() for k, v in f.items()}, n_const)
+        for k in f:
+            assert np.array_equal(fd[k].cpu().numpy().astype(np.float64), ref[k]), (k, n_const)

@@ -168,3 +168,27 @@ def test_pic_loop_keeps_the_wald_vacuum_stationary(O, W):
         err[(n, "late")] = max(rel(st["B"]), rel(st["D"]))
     assert err[(32, "late")] < 2.0 * err[(32, "early")] and err[(64, "late")] < 2.0 * err[(64, "early")], err   # bounded
     assert err[(32, "late")] < 0.1 and err[(64, "late")] < 0.6 * err[(32, "late")], err                           # converging
+
+
+def test_field_bc_leaves_an_axisymmetric_solution_unchanged(O, W):
+    """Axis reflection (Fig. 1): the analytic Wald field sampled on the Yee mesh INCLUDING its ghost columns
+    (signed sin(theta): the analytic continuation across the axis) already satisfies the reflection rules, so the
+    boundary condition must not change it: r- and phi-components even, theta-components odd, B^2 = D^3 = 0 on the
+    axes.  A wrong parity or a mirror index off by one changes the ghosts by O(1).  Constant layer."""
+    a = 0.9
+    dom = W.Domain(32, 16, a, 0.9 * W.horizon_radius(a), 20.0)
+    g = O.Grid(dom.n1, dom.n2, a, dom.r_min, dom.r_max)
+    f = W.wald_fields(dom, 1.0)
+    h = {k: np.array(v) for k, v in f.items()}
+    O.field_bc(g, h)
+    for k in f:
+        assert np.abs(h[k] - f[k]).max() <= 1e-9 * np.abs(f[k]).max(), k
+    rng = np.random.default_rng(2)
+    r = {k: rng.normal(size=g.shape) for k in f}
+    r0 = {k: v.copy() for k, v in r.items()}
+    O.field_bc(g, r, n_const=2)
+    G = g.ng
+    for k in r:
+        assert np.array_equal(r[k][G + 3:, G + 1:G + g.n2 - 1], r0[k][G + 3:, G + 1:G + g.n2 - 1])   # interior untouched
+        for row in range(G + 3):
+            assert np.array_equal(r[k][row], r[k][G + 3])                                           # layer = row n_f + 1
