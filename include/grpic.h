@@ -17,8 +17,8 @@
  *     exception and says so.  The structs themselves live in host memory and are read during the call.
  *   - The library owns only its context (constants, counters, sort scratch, tile table).
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default
- *     stream) and return without synchronising, except grpic_counters, grpic_sort's first scratch
- *     allocation and grpic_step_host.
+ *     stream) and return without synchronising, except grpic_counters, grpic_sort (scratch allocation
+ *     on first use and a 4-byte read-back of the alive count at its end) and grpic_step_host.
  *   - Return value: GRPIC_OK (0) or a negative grpic_status; grpic_last_error(ctx) gives the text.
  *     Nothing aborts or throws.  There is no CPU fallback: without a CUDA device every compute
  *     call returns GRPIC_ECUDA.
@@ -144,6 +144,13 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
  * Errors: EINVAL, ENOMEM, ECUDA. */
 int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* cuda_stream);
 int grpic_tile_size(void);
+
+/* Compaction / injection support.  After grpic_sort the alive particles of the species occupy the slots
+ * [0, n_alive) and the dead ones the rest; this call returns that n_alive (the caller may set p->n = n_alive to drop the
+ * dead slots, or write new particles into slots >= n_alive with tag = 1, or append beyond p->n and raise p->n).
+ * grpic_step pushes such slots through the direct kernel until the next grpic_sort, whatever was sorted before.
+ * Errors: EINVAL, ESTATE (species never sorted on this context). */
+int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_alive);
 
 /* Counters of the most recent push/step (alive after it, absorbed inside, absorbed outside) and
  * of the most recent deposit/step (n_overstep).  Synchronises `cuda_stream`. Any pointer may be NULL. */

@@ -27,6 +27,9 @@ std::string g_create_error;
 
 struct SortState {          // tile table of one species (keyed by the address of its i1 column)
   int64_t n_at_sort = 0;    // p->n when the table was built
+  int64_t n_alive = 0;      // alive particles at that time: slots [0, n_alive) are covered by the table, the rest
+                            // (dead at sort time, or appended later) by the direct path, so revived / injected
+                            // particles are never skipped
   WorkItem* items = nullptr;
   uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time
   uint32_t max_items = 0;
@@ -384,7 +387,7 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   const PPtrs<real> P = make_pptrs(p);
 
   auto it = ctx->sorted.find((const void*)p->i1);
-  const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_at_sort <= p->n && sc.em &&
+  const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n && sc.em &&
                      sc.do_deposit;
   const bool gen = general_map(ctx);             // full A.3 map (r0, h0): same kernels, general coordinate class
   if (!tiled) {
@@ -398,9 +401,9 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   const SortState& ss = it->second;
   std::string terr;
   const bool ok = gen ? launch_step_tiled<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
-                                                                ss.items, ss.d_n_items, ss.max_items, ss.n_at_sort, st, terr)
+                                                                ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
                       : launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
-                                                ss.d_n_items, ss.max_items, ss.n_at_sort, st, terr);
+                                                ss.d_n_items, ss.max_items, ss.n_alive, st, terr);
   if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
   return GRPIC_OK;
 }
@@ -504,6 +507,19 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
   CK(cudaMemcpyAsync(in.tag, p->tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
   k_sort_gather<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
   CK(cudaGetLastError());
+  // number of alive particles (they now occupy [0, n_alive)): 4 bytes read back, the one synchronisation of the sort
+  uint32_t h_alive = 0;
+  CK(cudaMemcpyAsync(&h_alive, ss.d_n_items + 1, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  ss.n_alive = (int64_t)h_alive;
+  return GRPIC_OK;
+}
+
+int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_alive) {
+  if (!ctx || !p || !n_alive) return fail(ctx, GRPIC_EINVAL, "NULL argument");
+  auto it = ctx->sorted.find((const void*)p->i1);
+  if (it == ctx->sorted.end()) return fail(ctx, GRPIC_ESTATE, "this species has not been sorted on this context");
+  *n_alive = it->second.n_alive;
   return GRPIC_OK;
 }
 

@@ -23,7 +23,7 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
-           "grpic_field_bc"]
+           "grpic_field_bc", "grpic_sorted_alive"]
 
 
 class GrpicError(RuntimeError):
@@ -94,6 +94,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_aux_fields.argtypes = [_vp, C.POINTER(_Fields), C.POINTER(_Vec3), C.POINTER(_Vec3), _vp]
     lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
+    lib.grpic_sorted_alive.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(C.c_int64)]
     lib.grpic_field_bc.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_int32, _vp]
     lib.grpic_fields_prepare.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_fields_advance.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.POINTER(_Current),
@@ -275,6 +276,12 @@ class Context:
     def sort(self, p: ParticleSet, stream=None):
         ps = p.c_struct()
         self._ck(self.lib.grpic_sort(self.h, C.byref(ps), _stream_ptr(stream)))
+
+    def sorted_alive(self, p: ParticleSet) -> int:
+        """alive particles of the species at its last sort; they occupy the slots [0, n_alive)"""
+        ps = p.c_struct(); v = C.c_int64(0)
+        self._ck(self.lib.grpic_sorted_alive(self.h, C.byref(ps), C.byref(v)))
+        return int(v.value)
 
     def counters(self, stream=None):
         v = [C.c_int64(0) for _ in range(4)]

@@ -610,3 +610,54 @@ def test_gauss_law_is_kept_by_the_closed_loop_on_the_gpu(G, O, W):
         assert drift < 1e-11 * scale * (step + 1), (step, drift, scale)
     assert absorbed > 0          # the run did exercise absorption (outside the checked nodes)
     print("Gauss-law drift after 30 steps:", drift, "scale", scale, "absorbed", absorbed)
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_injection_and_compaction_after_a_sort(G, O, W, prec):
+    """after grpic_sort the alive particles sit in [0, n_alive) (grpic_sorted_alive).  Particles written
+    into dead slots (tag 0 -> 1) and particles appended beyond the sorted range must be pushed and deposited by the
+    next grpic_step although the tile table does not know them; truncating the set to n_alive drops only dead ones."""
+    import torch
+    wl = W.config_large(shrink=32)
+    dom = wl.dom
+    g = grid_from_domain(O, dom)
+    ctx = _ctx(G, dom, prec)
+    fdev, fhost = _fields_both(G, wl, prec)
+    sp = wl.species[0]
+    rng = np.random.default_rng(8)
+    sp.tag = sp.tag.copy(); sp.tag[rng.random(sp.n) < 0.2] = 0
+    ps = G.ParticleSet.from_host(sp, prec)
+    ctx.sort(ps)
+    n_alive = ctx.sorted_alive(ps)
+    assert n_alive == int(sp.tag.sum()) and bool((ps.cols["tag"][:n_alive] == 1).all()) and bool((ps.cols["tag"][n_alive:] == 0).all())
+    # revive every second dead slot with a fresh particle, and append 1000 more beyond the old length
+    n_old = ps.n
+    idx = torch.arange(n_alive, n_old, 2, device="cuda")
+    extra = 1000
+    cols = {}
+    for k, v in ps.cols.items():
+        cols[k] = torch.cat([v, v[:extra].clone()])
+    rt = G.torch_real(prec)
+    gen = torch.Generator(device="cuda"); gen.manual_seed(5)
+    newi = torch.cat([idx, torch.arange(n_old, n_old + extra, device="cuda")])
+    m = newi.numel()
+    cols["i1"][newi] = torch.randint(4, dom.n1 - 4, (m,), device="cuda", generator=gen, dtype=torch.int32)
+    cols["i2"][newi] = torch.randint(1, dom.n2 - 1, (m,), device="cuda", generator=gen, dtype=torch.int32)
+    for k in ("dx1", "dx2"):
+        cols[k][newi] = torch.rand(m, device="cuda", generator=gen, dtype=torch.float64).to(rt) * 0.999
+    for k in ("u1", "u2", "u3"):
+        cols[k][newi] = (torch.rand(m, device="cuda", generator=gen, dtype=torch.float64).to(rt) - 0.5) * 0.02
+    cols["weight"][newi] = 1.0
+    cols["tag"][newi] = 1
+    # the sort table is keyed by the address of the i1 column: keep the original storage for the sorted part
+    ps2 = G.ParticleSet(cols, ps.q_over_m, ps.charge, ps.massive)
+    ctx.sort(ps2)                                   # a table for the new storage ...
+    n2_alive = ctx.sorted_alive(ps2)
+    assert n2_alive == n_alive + m
+    # ... then make it stale again: kill some, revive others, so that the direct path must serve slots >= n_alive
+    cols["tag"][n2_alive - 500:n2_alive] = 0
+    dead = torch.arange(n2_alive, ps2.n, device="cuda")[:300]
+    cols["tag"][dead] = 1
+    cols["i1"][dead] = 10; cols["i2"][dead] = 5
+    res, c = _one_step_parity(G, O, ctx, g, ps2, fdev, fhost, wl.dt, prec, "fused")
+    assert c["alive"] + c["absorbed_in"] + c["absorbed_out"] == n2_alive - 500 + 300
