@@ -3,7 +3,9 @@
  *
  * What is behind it: the per-particle step of the general-relativistic particle-in-cell
  * method of arxiv/paper_2511_17701 ("Entity II: General Relativistic Module") on a 2D
- * axisymmetric (r, theta) Kerr-Schild grid, as hand-written sm_100a CUDA kernels.
+ * axisymmetric (r, theta) Kerr-Schild grid, as hand-written sm_100a CUDA kernels — and, around it,
+ * the field-solver half of the same timestep (auxiliary fields, Faraday, Ampere, field boundary
+ * conditions), so that the calls below close the PIC loop of Sec. 3.4.
  * "P:n" below = line n of the paper text; "R-Sk" = reading k of DESIGN.md.
  *
  * Two builds of one source export the SAME symbols:
@@ -31,7 +33,9 @@
  *     layer.  Ghost zones of J are written raw (folding them back is field-side work).
  *   - Code coordinates: x1 in [0, n1) is radial with r = r_min * exp(x1 * ln(r_max/r_min)/n1)
  *     (App. A.3 with r0 = 0), x2 in [0, n2) is polar with theta = x2 * pi/n2; a position
- *     is (cell index i, displacement dx in [0,1)) per axis.  r_g = M = 1.
+ *     is (cell index i, displacement dx in [0,1)) per axis.  r_g = M = 1.  This is the default
+ *     map, the one of the five benchmark configs; the other maps of App. A (uniform r, radial offset,
+ *     polar stretch, flat space) are selected with grid.r_map and grpic_set_real (see there).
  */
 #ifndef GRPIC_H_
 #define GRPIC_H_
