@@ -24,7 +24,10 @@ constexpr int kRowF = kWinF + 4;                // shared row length of the fiel
                                                 // column 16-byte aligned in global memory, so up to 3 extra
                                                 // columns are fetched on the left              (28)
 constexpr int kWinJ = kWinC + 1;                // J nodes per window edge: c .. c+1         (23)
-constexpr int kChunk = 4096;                    // max particles per work item
+#ifndef GRPIC_CHUNK
+#define GRPIC_CHUNK 16384
+#endif
+constexpr int kChunk = GRPIC_CHUNK;             // max particles per work item
 constexpr int kBlock = 256;
 
 template <typename T>
