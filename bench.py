@@ -107,6 +107,16 @@ def _oracle_step(O, wl, g, parts, fields):
     return n
 
 
+def _cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(name, shrink=16, steps=1):
     O, wl, g, parts, fields = _oracle_setup(name, shrink)
     t0 = time.perf_counter()
@@ -114,7 +124,16 @@ def cpu_baseline(name, shrink=16, steps=1):
     for _ in range(steps):
         n += _oracle_step(O, wl, g, parts, fields)
     dt = time.perf_counter() - t0
-    return {"value": n / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+    # one single-thread figure on a smaller sample
+    nt = O.num_threads()
+    O1, wl1, g1, parts1, fields1 = _oracle_setup(name, shrink * 2)
+    O.set_num_threads(1)
+    t1 = time.perf_counter()
+    n1 = _oracle_step(O1, wl1, g1, parts1, fields1)
+    dt1 = time.perf_counter() - t1
+    O.set_num_threads(nt)
+    return {"value": n / dt, "unit": UNIT, "cores": nt, "kind": "oracle", "cpu_model": _cpu_model(),
+            "single_thread_value": n1 / dt1,
             "sample": f"{steps} step(s) of {_workload_desc(wl, shrink)}; oracle = oracle/grpic_oracle.c "
                       f"(FP64, OpenMP over particles), {dt:.1f} s"}
 
@@ -340,6 +359,8 @@ def run_ours(args):
                      "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                              "frac": hbm_ach / peaks["hbm_gbs"], "bytes_per_update": BYTES_PER_UPDATE[prec],
                              "peak_source": peak_src}},
+        "without_sort": {"value": updates / (step_kernel_ms * 1e-3), "unit": UNIT,
+                         "note": "fused step launches only (CUDA events around each launch); `value` includes grpic_sort every sort_every steps and the J zero-fills"},
         "clocks": clocks, "gpu_launches": launches,
         "counters_last_step": counters, "updates_timed": updates_all,
     }
