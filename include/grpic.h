@@ -193,6 +193,12 @@ int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic
  * (paper I) is not part of this call.  Errors: EINVAL, ECUDA. */
 int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const, void* cuda_stream);
 
+/* Current filter ("n_f passes of a digital filter"; the paper defers its form to paper I — reading R-F5 of
+ * DESIGN.md): n_passes of the binomial smoothing [1 2 1]/4 along x2 and along x1, in place on J, each component on its
+ * own Yee lattice; mirror samples with the component's parity beyond the polar axes; the first and last array rows are
+ * not smoothed along x1.  Errors: EINVAL, ENOMEM (scratch), ECUDA. */
+int grpic_filter_current(grpic_ctx* ctx, grpic_current* J, int32_t n_passes, void* cuda_stream);
+
 /* Field side of one PIC timestep (Sec. 3.4), built from the three operations above.  The state holds
  * (n-3/2)B, (n-1/2)B, (n-1)D, (n)D; all arrays caller-owned device memory; library scratch: 12 grid arrays.
  *   grpic_fields_prepare  step 2, Eq. 46-48: B_n <- (n)B, the magnetic field aligned in time with (n)D for the push

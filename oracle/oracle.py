@@ -396,3 +396,32 @@ def field_bc(g: Grid, fields: dict, n_const: int = -1) -> dict:
         for A in fields.values():
             A[: G + n_const + 1, :] = A[G + n_const + 1, :]
     return fields
+
+
+# ----------------------------------------------------------------------------------------------
+# Current filter ("n_f passes of a digital filter", details deferred to paper I).  Reading R-F5: the
+# standard binomial 1-2-1 smoothing of PIC codes, separable in x1 and x2, one pass = [1 2 1]/4 along each axis, on
+# each component's own Yee lattice; beyond the polar axes the neighbour is the mirror sample with the component's
+# parity (J^1, J^3 even, J^2 odd, as D^i); the first and last array rows are left as they are.
+# The CHOICE of filter is parity unpinned (any symmetric normalised stencil commutes with the continuity equation).
+# ----------------------------------------------------------------------------------------------
+_J_PARITY = {"J1": (+1, 0.0), "J2": (-1, 0.5), "J3": (+1, 0.0)}
+
+
+def filter_current(g: Grid, J: dict, n_passes: int = 1) -> dict:
+    G, n2 = g.ng, g.n2
+    for _ in range(int(n_passes)):
+        for k, (par, off) in _J_PARITY.items():
+            A = J[k]
+            ncol = n2 + 1 if off == 0.0 else n2                 # physical samples in theta
+            P = np.zeros((A.shape[0], ncol + 2))
+            P[:, 1:-1] = A[:, G:G + ncol]
+            if off == 0.0:                                      # node-sampled: j = -1 mirrors j = +1, n2+1 mirrors n2-1
+                P[:, 0] = par * A[:, G + 1]; P[:, -1] = par * A[:, G + n2 - 1]
+            else:                                               # half-sampled: -1/2 mirrors +1/2, n2+1/2 mirrors n2-1/2
+                P[:, 0] = par * A[:, G]; P[:, -1] = par * A[:, G + n2 - 1]
+            T = 0.25 * (P[:, :-2] + 2.0 * P[:, 1:-1] + P[:, 2:])               # along x2
+            out = T.copy()
+            out[1:-1] = 0.25 * (T[:-2] + 2.0 * T[1:-1] + T[2:])                # along x1, edge rows unchanged in x1
+            A[:, G:G + ncol] = out
+    return J

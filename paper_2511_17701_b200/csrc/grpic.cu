@@ -633,6 +633,29 @@ void average3(real* out, const real* a1, const real* a2, const real* a3, const r
 }
 }  // namespace
 
+int grpic_filter_current(grpic_ctx* ctx, grpic_current* J, int32_t n_passes, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!J || !J->J1 || !J->J2 || !J->J3) return fail(ctx, GRPIC_EINVAL, "a current component pointer is NULL");
+  if (n_passes < 0) return fail(ctx, GRPIC_EINVAL, "n_passes must be >= 0");
+  const FieldGeom q = make_field_geom(ctx);
+  if (q.n2 < 2) return fail(ctx, GRPIC_EINVAL, "n2 must be >= 2 for the filter");
+  const size_t cells = (size_t)q.rows * q.ld, bytes = cells * sizeof(real);
+  int rc = field_scratch(ctx, cells);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  real* S = ctx->f_scratch;
+  real* Jp[3] = {J->J1, J->J2, J->J3};
+  for (int pass = 0; pass < n_passes; ++pass) {
+    // scratch <- J (ghost columns and all), then J <- filter(scratch) on the physical samples
+    for (int c = 0; c < 3; ++c) CK(cudaMemcpyAsync(S + c * cells, Jp[c], bytes, cudaMemcpyDeviceToDevice, st));
+    CV3<real> in{{S, S + cells, S + 2 * cells}};
+    V3<real> out{{Jp[0], Jp[1], Jp[2]}};
+    k_filter_current<real><<<dim3((q.n2 + 1 + 127) / 128, q.rows, 3), 128, 0, st>>>(q, in, out);
+  }
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
 int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3* B_n, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
   if (!s || !vec3_ok(&s->B_prev) || !vec3_ok(&s->B) || !vec3_ok(&s->D_prev) || !vec3_ok(&s->D) || !vec3_ok(B_n))

@@ -207,6 +207,30 @@ __global__ void __launch_bounds__(128) k_field_bc_layer(const FieldGeom q, const
   A[(int64_t)a1 * q.ld + a2] = A[(int64_t)(q.ng + n_const + 1) * q.ld + a2];
 }
 
+// One pass of the binomial current filter (reading R-F5): [1 2 1]/4 along x2 then along x1 on the
+// component's own Yee lattice, mirror samples with the component's parity beyond the axes (J^1, J^3 even, J^2 odd),
+// first and last array row unchanged along x1.  in -> out (different arrays); one thread per (row, theta sample).
+template <typename T>
+__global__ void __launch_bounds__(128) k_filter_current(const FieldGeom q, const CV3<T> in, const V3<T> out) {
+  const int c = blockIdx.z, a1 = blockIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool half = (c == 1);
+  const int ncol = half ? q.n2 : q.n2 + 1;
+  if (j >= ncol) return;
+  const T par = (c == 1) ? T(-1) : T(1);
+  const T* A = in.f[c];
+  auto theta_pass = [&](int row) {
+    const T* r = A + (int64_t)row * q.ld + q.ng;
+    T lo, hi;
+    if (j > 0) lo = r[j - 1]; else lo = par * (half ? r[0] : r[1]);
+    if (j < ncol - 1) hi = r[j + 1]; else hi = par * (half ? r[q.n2 - 1] : r[q.n2 - 1]);
+    return T(0.25) * (lo + T(2) * r[j] + hi);
+  };
+  const T mid = theta_pass(a1);
+  T v = mid;
+  if (a1 > 0 && a1 < q.rows - 1) v = T(0.25) * (theta_pass(a1 - 1) + T(2) * mid + theta_pass(a1 + 1));
+  out.f[c][(int64_t)a1 * q.ld + q.ng + j] = v;
+}
+
 // out = (a + b)/2 over whole arrays (the time averages of Eq. 46 and Eq. 51)
 template <typename T>
 __global__ void __launch_bounds__(256) k_average(T* out, const T* a, const T* b, int64_t n) {

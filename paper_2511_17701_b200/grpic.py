@@ -23,7 +23,7 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
-           "grpic_field_bc", "grpic_sorted_alive"]
+           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current"]
 
 
 class GrpicError(RuntimeError):
@@ -95,6 +95,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
     lib.grpic_sorted_alive.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(C.c_int64)]
+    lib.grpic_filter_current.argtypes = [_vp, C.POINTER(_Current), C.c_int32, _vp]
     lib.grpic_field_bc.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_int32, _vp]
     lib.grpic_fields_prepare.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_fields_advance.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.POINTER(_Current),
@@ -322,6 +323,10 @@ class Context:
         js = _current_struct(J)
         self._ck(self.lib.grpic_ampere(self.h, C.byref(d), C.byref(h), C.byref(js) if js else None, float(dt),
                                        _stream_ptr(stream)))
+
+    def filter_current(self, J, n_passes=1, stream=None):
+        js = _current_struct(J)
+        self._ck(self.lib.grpic_filter_current(self.h, C.byref(js), int(n_passes), _stream_ptr(stream)))
 
     def field_bc(self, fields, n_const=-1, stream=None):
         """Axis reflection of the ghost columns, zeros on the axes, constant layer inside the horizon (in place)."""

@@ -661,3 +661,22 @@ def test_injection_and_compaction_after_a_sort(G, O, W, prec):
     cols["i1"][dead] = 10; cols["i2"][dead] = 5
     res, c = _one_step_parity(G, O, ctx, g, ps2, fdev, fhost, wl.dt, prec, "fused")
     assert c["alive"] + c["absorbed_in"] + c["absorbed_out"] == n2_alive - 500 + 300
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_filter_current(G, O, W, prec):
+    """grpic_filter_current against the oracle (1 and 3 passes) on random currents; ghost columns untouched."""
+    import torch
+    g = O.Grid(37, 150, 0.9, 1.3, 15.0, ng=2)
+    ctx = G.Context(g.n1, g.n2, 0.9, g.r_min, g.r_max, nghost=2, precision=prec)
+    rng = np.random.default_rng(4)
+    rt = np.float32 if prec == "f32" else np.float64
+    J = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in ("J1", "J2", "J3")}
+    for n in (1, 3):
+        Jd = {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in J.items()}
+        ctx.filter_current(Jd, n)
+        ref = O.filter_current(g, {k: v.copy() for k, v in J.items()}, n)
+        for k in J:
+            got = Jd[k].cpu().numpy().astype(np.float64)
+            assert np.abs(got - ref[k]).max() <= (2e-6 if prec == "f32" else 1e-14), (k, n)
+            assert np.array_equal(got[:, :2], J[k][:, :2])

@@ -192,3 +192,38 @@ def test_field_bc_leaves_an_axisymmetric_solution_unchanged(O, W):
         assert np.array_equal(r[k][G + 3:, G + 1:G + g.n2 - 1], r0[k][G + 3:, G + 1:G + g.n2 - 1])   # interior untouched
         for row in range(G + 3):
             assert np.array_equal(r[k][row], r[k][G + 3])                                           # layer = row n_f + 1
+
+
+def test_current_filter_properties(O):
+    """Binomial filter (reading R-F5): constants are invariant, the Nyquist mode along x1 is annihilated in one pass,
+    n passes along x1 are the convolution with the binomial coefficients C(2n, k)/4^n, the filter commutes with the
+    difference operators of the continuity equation (so a filtered rho keeps Gauss's law), and it respects the axis
+    parities (an odd J^2 stays odd: its mirror-extended sum across the axis vanishes)."""
+    from math import comb
+    g = O.Grid(24, 16, 0.9, 1.3, 15.0)
+    G = g.ng
+    J = {k: np.full(g.shape, 3.0) for k in ("J1", "J2", "J3")}
+    J["J2"][:] = 0.0                                                      # a constant J^2 is not odd across the axis
+    O.filter_current(g, J, 2)
+    assert np.allclose(J["J1"][:, G:G + g.n2 + 1], 3.0) and np.allclose(J["J3"][:, G:G + g.n2 + 1], 3.0)
+    alt = ((-1.0) ** np.arange(g.shape[0]))[:, None] * np.ones(g.shape)
+    J = {k: alt.copy() for k in ("J1", "J2", "J3")}
+    O.filter_current(g, J, 1)
+    assert np.abs(J["J1"][1:-1, G + 1:G + g.n2]).max() < 1e-15            # Nyquist along x1 gone
+    rng = np.random.default_rng(1)
+    n = 3
+    d = np.zeros(g.shape); d[12, G + 7] = 1.0
+    J = {"J1": d.copy(), "J2": np.zeros(g.shape), "J3": np.zeros(g.shape)}
+    O.filter_current(g, J, n)
+    coef = np.array([comb(2 * n, k) for k in range(2 * n + 1)]) / 4.0 ** n
+    assert np.allclose(J["J1"][12 - n:12 + n + 1, G + 7] / J["J1"][12, G + 7], coef / coef[n], rtol=1e-13)
+    assert np.isclose(J["J1"].sum(), 1.0, rtol=1e-13)                     # total current kept
+    # commutes with the x1 difference in the interior
+    A = rng.normal(size=g.shape)
+    J1 = {"J1": A.copy(), "J2": np.zeros(g.shape), "J3": np.zeros(g.shape)}
+    O.filter_current(g, J1, 1)
+    dA = np.zeros(g.shape); dA[1:] = A[1:] - A[:-1]
+    J2 = {"J1": dA.copy(), "J2": np.zeros(g.shape), "J3": np.zeros(g.shape)}
+    O.filter_current(g, J2, 1)
+    lhs = J1["J1"][3:-2, G:G + g.n2 + 1] - J1["J1"][2:-3, G:G + g.n2 + 1]
+    assert np.allclose(lhs, J2["J1"][3:-2, G:G + g.n2 + 1], atol=1e-13)
