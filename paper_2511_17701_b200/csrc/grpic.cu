@@ -360,6 +360,19 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
   cudaStream_t st = (cudaStream_t)stream;
   CK(cudaMemsetAsync(ctx->d_counters + 3, 0, sizeof(unsigned long long), st));
   if (p->n == 0 || !sc.do_deposit) return GRPIC_OK;
+  auto it = ctx->sorted.find((const void*)p->i1);
+  if (ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n) {
+    // sorted species: per-warp shared J tiles and warp aggregation instead of one L2 reduction per contribution
+    const SortState& ss = it->second;
+    std::string terr;
+    const bool ok = general_map(ctx)
+        ? launch_deposit_tiled<real, CoordGen<real>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items,
+                                                     ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
+        : launch_deposit_tiled<real>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items, ss.d_n_items,
+                                     ss.max_items, ss.n_alive, st, terr);
+    if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
+    return GRPIC_OK;
+  }
   if (general_map(ctx))
     k_deposit<real, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters);
   else

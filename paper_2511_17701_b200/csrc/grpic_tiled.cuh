@@ -506,6 +506,142 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// grpic_deposit over the sorted tiles: the deposit of (prev -> current) with the same per-warp private J tiles, warp
+// aggregation and straggler queue as the fused step (steps 4-5 above); no field staging.  Items are the tiles of the
+// last grpic_sort; the window test uses the PREVIOUS cell (the start of the path), like the fused kernel.
+// The direct k_deposit sends every contribution to L2 with red.global.add: 13.5 ms for the 67 M particles of
+// config 4 (hundreds of particles per cell hitting the same addresses); this kernel: see DESIGN.md section 7.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+constexpr size_t deposit_smem_bytes() {
+  return (size_t)(kJElems + kWarps * kQueueVals) * sizeof(T) + (size_t)kWarps * kQueue * sizeof(int);
+}
+
+template <typename T, typename CoordT = Coord<T>>
+__global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 2))
+    k_deposit_tiled(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J, const SpeciesConst sc,
+                    unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr, uint32_t max_items,
+                    int64_t n_covered, int nt2) {
+  extern __shared__ __align__(128) unsigned char smem_raw_[];
+  T* sF = reinterpret_cast<T*>(smem_raw_);
+  T* sQv = sF + kJElems;
+  int* sQk = reinterpret_cast<int*>(sQv + kWarps * kQueueVals);
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  T* sJ = sF + wid * kJTile;
+  const T eps = sc.massive ? T(1) : T(0);
+  const T inv_dt = T(1) / (T)sc.dt;
+  const T chg = (T)sc.charge;
+  unsigned n_over = 0;
+
+  auto one = [&](int64_t k, bool in_window_ok, int c1lo, int c2lo, bool& dep_a, int& node_a, bool& dep_b, int& node_b,
+                 T seg[2][8]) {
+    dep_a = dep_b = false; node_a = node_b = 0;
+    if (k >= P.n || P.tag[k] == 0) return;
+    const int ia = P.i1p[k], ja = P.i2p[k];
+    const int di = P.i1[k] - ia, dj = P.i2[k] - ja;
+    if (di > 1 || di < -1 || dj > 1 || dj < -1) { ++n_over; return; }
+    const T xa = P.dx1p[k], ya = P.dx2p[k], dx1 = P.dx1[k], dx2 = P.dx2[k];
+    const T v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + dx1), T(0.5) * (ya + (T)dj + dx2),
+                                                P.u1[k], P.u2[k], P.u3[k], eps);
+    const T qw = chg * P.w[k];
+    deposit_segments(di, dj, xa, ya, dx1, dx2, qw * inv_dt, qw, v3, seg);
+    const bool cross = (di != 0) || (dj != 0);
+    if (!cross) {
+#pragma unroll
+      for (int q = 0; q < 8; ++q) seg[0][q] += seg[1][q];
+    }
+    const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
+    const int wa1 = ia - c1lo, wa2 = ja - c2lo, wb1 = wa1 + di, wb2 = wa2 + dj;
+    const bool a_in = in_window_ok && (unsigned)wa1 < (unsigned)kWinC && (unsigned)wa2 < (unsigned)kWinC;
+    const bool b_in = in_window_ok && (unsigned)wb1 < (unsigned)kWinC && (unsigned)wb2 < (unsigned)kWinC;
+    if (a_in && b_in) {
+      dep_a = true; dep_b = cross;
+      node_a = wa1 * kJStride + wa2; node_b = wb1 * kJStride + wb2;
+    } else {
+      global_add8(J, cell, g.ld, seg[0]);
+      if (cross) global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
+    }
+  };
+
+  if (blockIdx.x >= max_items) {                      // slots the table does not cover: straight to L2
+    const int64_t k = n_covered + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
+    bool da, db; int na, nb; T seg[2][8];
+    one(k, false, 0, 0, da, na, db, nb, seg);
+    if (n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
+    return;
+  }
+  if (blockIdx.x >= n_items_ptr[0]) return;
+  const WorkItem item = items[blockIdx.x];
+  const int c1lo = (int)(item.tile / (uint32_t)nt2) * kTile - kHalo;
+  const int c2lo = (int)(item.tile % (uint32_t)nt2) * kTile - kHalo;
+  {
+    float4* z4 = reinterpret_cast<float4*>(sF);
+    constexpr int n4 = (int)(kJElems * sizeof(T) / 16);
+    for (int e = tid; e < n4; e += kTBlock) z4[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncthreads();
+  const int my_off = j_offset_of(((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1));
+  WarpQueue<T> Q{sQk + wid * kQueue, sQv + wid * kQueueVals, 0};
+  const uint32_t end = item.begin + item.count;
+  const uint32_t per_warp = ((item.count + kTBlock - 1) / kTBlock) * 32u;
+  const uint32_t w_begin = item.begin + (uint32_t)wid * per_warp;
+  const uint32_t w_end = min(end, w_begin + per_warp);
+  for (uint32_t base = w_begin; base < w_end; base += 32u) {
+    const uint32_t k = base + lane;
+    bool dep_a, dep_b; int node_a, node_b; T seg[2][8];
+    one(k < w_end ? (int64_t)k : (int64_t)P.n, true, c1lo, c2lo, dep_a, node_a, dep_b, node_b, seg);
+    const bool left_a = warp_deposit<T, false>(sJ, lane, my_off, dep_a, node_a, seg[0]);
+    Q.append(lane, left_a, node_a, seg[0]);
+    Q.drain(sJ, lane, my_off, 31);
+    Q.append(lane, dep_b, node_b, seg[1]);
+    Q.drain(sJ, lane, my_off, 31);
+  }
+  Q.drain(sJ, lane, my_off, 0);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) n_over += __shfl_xor_sync(0xffffffffu, n_over, o);
+  if (lane == 0 && n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
+  __syncthreads();
+  const int rows = g.n1 + 2 * g.ng;
+  for (int e = tid; e < kJTile; e += kTBlock) {
+    T v = sF[e];
+#pragma unroll
+    for (int q = 1; q < kWarps; ++q) v += sF[q * kJTile + e];
+    if (v != T(0)) {
+      const int c = e / kJComp, rem = e % kJComp;
+      const int a1 = c1lo + g.ng + rem / kJStride, a2 = c2lo + g.ng + rem % kJStride;
+      if (a1 >= 0 && a1 < rows && a2 >= 0 && a2 < g.ld) red_add(J.j[c] + (int64_t)a1 * g.ld + a2, v);
+    }
+  }
+}
+
+template <typename T, typename CoordT = Coord<T>>
+bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>& J, const SpeciesConst& sc,
+                          unsigned long long* counters, const WorkItem* items, const uint32_t* d_n_items,
+                          uint32_t max_items, int64_t n_covered, cudaStream_t st, std::string& err) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t ea = cudaFuncSetAttribute(k_deposit_tiled<T, CoordT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)deposit_smem_bytes<T>());
+    if (ea != cudaSuccess) {
+      err = std::string("k_deposit_tiled shared-memory opt-in: ") + cudaGetErrorString(ea);
+      return false;
+    }
+    attr_set = true;
+  }
+  const int nt2 = (g.n2 + kTile - 1) / kTile;
+  const int64_t tail = P.n > n_covered ? P.n - n_covered : 0;
+  const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
+  k_deposit_tiled<T, CoordT><<<grid, kTBlock, deposit_smem_bytes<T>(), st>>>(g, P, J, sc, counters, items, d_n_items,
+                                                                            max_items, n_covered, nt2);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    err = std::string("k_deposit_tiled launch: ") + cudaGetErrorString(e);
+    return false;
+  }
+  return true;
+}
+
 template <typename T, typename CoordT = Coord<T>>
 bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,

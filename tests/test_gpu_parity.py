@@ -141,7 +141,7 @@ def _shrunk(W, name, shrink):
 
 @pytest.mark.parametrize("name,shrink,prec", [("magnetosphere", 8, "f32"), ("large", 16, "f32"),
                                               ("two_species", 8, "f64"), ("two_species", 8, "f32")])
-@pytest.mark.parametrize("mode", ["split", "fused", "tiled"])
+@pytest.mark.parametrize("mode", ["split", "fused", "tiled", "tiled_split"])
 def test_configs_3_4_5_shrunk(G, O, W, name, shrink, prec, mode):
     """Configs 3-5 with both grid edges divided by `shrink` (per-cell counts, fields, dt recipe kept):
     several tiles and a ragged tail; 3 steps per species."""
@@ -153,8 +153,10 @@ def test_configs_3_4_5_shrunk(G, O, W, name, shrink, prec, mode):
     worst = {}
     for step in range(3):
         for ps in sets:
+            # "tiled": sort, then the fused tile kernel; "tiled_split": sort, then grpic_interp_push + the tiled grpic_deposit
             res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, prec,
-                                      "fused" if mode == "tiled" else mode, sort_first=(mode == "tiled" and step == 0))
+                                      {"tiled": "fused", "tiled_split": "split"}.get(mode, mode),
+                                      sort_first=(mode.startswith("tiled") and step == 0))
             for k, v in res.items():
                 worst[k] = max(worst.get(k, 0), v)
     print(name, prec, mode, worst)
