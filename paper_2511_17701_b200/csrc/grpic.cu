@@ -339,6 +339,23 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
   CK(cudaMemsetAsync(ctx->d_counters, 0, 3 * sizeof(unsigned long long), st));
   if (p->n == 0) return GRPIC_OK;
   JPtrs<real> J{{nullptr, nullptr, nullptr}};
+  {
+    auto it = ctx->sorted.find((const void*)p->i1);
+    if (ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n && sc.em) {
+      // sorted species: field stencil of each tile staged in shared memory, as in the fused step
+      const SortState& ss = it->second;
+      std::string terr;
+      const Consts<real> g = make_consts(ctx);
+      const PPtrs<real> P = make_pptrs(p);
+      const bool ok = general_map(ctx)
+          ? launch_step_tiled<real, CoordGen<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
+                                                           ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
+          : launch_step_tiled<real, Coord<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
+                                                        ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr);
+      if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
+      return GRPIC_OK;
+    }
+  }
   if (general_map(ctx))
     k_push_or_step<real, false, CoordGen<real>><<<grid_for(p->n), kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), F, J, sc,
                                                                                    ctx->d_counters);

@@ -300,7 +300,8 @@ struct RawAcc {      // raw staged stencil: sample (row, col) of component c
   }
 };
 
-template <typename T, typename CoordT = Coord<T>>
+// kDeposit = false is grpic_interp_push over the sorted tiles: the same kernel without steps 4-5.
+template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
@@ -318,7 +319,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   // ---- tail blocks: particles appended after the last sort -> direct path ----
   if (blockIdx.x >= max_items) {
     const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
-    particle_direct<T, true, CoordT>(g, P, F, J, sc, counters, k);
+    particle_direct<T, kDeposit, CoordT>(g, P, F, J, sc, counters, k);
     return;
   }
   if (blockIdx.x >= n_items_ptr[0]) return;
@@ -437,7 +438,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
       P.u1[k] = p.u1; P.u2[k] = p.u2; P.u3[k] = p.u3;
       if (sc.has_phi) P.phi[k] = phi + dt * dphidt;
       if (res != 0) P.tag[k] = 0;
-      if (res == 0) {
+      if (kDeposit && res == 0) {
         const int di = p.i1 - ia, dj = p.i2 - ja;
         if (di > 1 || di < -1 || dj > 1 || dj < -1) {
           ++n_over;
@@ -468,14 +469,16 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
       }
       n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
     }
-    // big groups of the start cells now; stragglers and the neighbour-cell parts through the queue
-    const bool left_a = warp_deposit<T, false>(sJ, lane, my_off, dep_a, node_a, seg[0]);
-    Q.append(lane, left_a, node_a, seg[0]);
-    Q.drain(sJ, lane, my_off, 31);
-    Q.append(lane, dep_b, node_b, seg[1]);
-    Q.drain(sJ, lane, my_off, 31);
+    if (kDeposit) {
+      // big groups of the start cells now; stragglers and the neighbour-cell parts through the queue
+      const bool left_a = warp_deposit<T, false>(sJ, lane, my_off, dep_a, node_a, seg[0]);
+      Q.append(lane, left_a, node_a, seg[0]);
+      Q.drain(sJ, lane, my_off, 31);
+      Q.append(lane, dep_b, node_b, seg[1]);
+      Q.drain(sJ, lane, my_off, 31);
+    }
   }
-  Q.drain(sJ, lane, my_off, 0);
+  if (kDeposit) Q.drain(sJ, lane, my_off, 0);
   // counters: one atomic per warp and counter
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -491,6 +494,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
     if (n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
     if (n_alive + n_in + n_out) atomicAdd(&counters[4], (unsigned long long)(n_alive + n_in + n_out));
   }
+  if (!kDeposit) return;
   // ---- 5. flush: sum the private tiles, one reduction per touched entry ----
   __syncthreads();
   const int rows = g.n1 + 2 * g.ng;
@@ -642,14 +646,14 @@ bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>&
   return true;
 }
 
-template <typename T, typename CoordT = Coord<T>>
+template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
                        const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
                        cudaStream_t st, std::string& err) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T, CoordT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T, CoordT, kDeposit>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)tiled_smem_bytes<T>());
     if (ea != cudaSuccess) {
       err = std::string("k_step_tiled shared-memory opt-in: ") + cudaGetErrorString(ea);
@@ -666,7 +670,7 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   const int nt2 = (g.n2 + kTile - 1) / kTile;
   const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
   const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
-  k_step_tiled<T, CoordT><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
+  k_step_tiled<T, CoordT, kDeposit><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
                                                                 n_at_sort, nt2, use_tma, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
