@@ -170,7 +170,7 @@ __device__ __forceinline__ void private_add8(T* sJ, bool on, int node, const T v
 //   - The lanes of smaller groups are served by rank inside their group: round r takes the r-th lane of
 //     every group, so the lanes of one round hold pairwise different cells (private_add8).
 #ifndef GRPIC_BIG_GROUP
-#define GRPIC_BIG_GROUP 4
+#define GRPIC_BIG_GROUP 6
 #endif
 constexpr int kBigGroup = GRPIC_BIG_GROUP;
 
