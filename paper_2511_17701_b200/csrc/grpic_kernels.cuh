@@ -17,12 +17,15 @@
 namespace grpic {
 
 constexpr int kTile = 16;                       // cells per tile edge (sort key and shared-memory tile)
-constexpr int kHalo = 3;                        // extra cells around a tile served from shared memory
+#ifndef GRPIC_HALO
+#define GRPIC_HALO 3
+#endif
+constexpr int kHalo = GRPIC_HALO;               // extra cells around a tile served from shared memory
 constexpr int kWinC = kTile + 2 * kHalo;        // cells per window edge                     (22)
 constexpr int kWinF = kWinC + 2;                // field samples per window edge: c-1 .. c+1 (24)
-constexpr int kRowF = kWinF + 4;                // shared row length of the field window: TMA wants the first
-                                                // column 16-byte aligned in global memory, so up to 3 extra
-                                                // columns are fetched on the left              (28)
+constexpr int kRowF = (kWinF + 3 + 3) / 4 * 4;  // shared row length of the field window: TMA wants the first
+                                                // column 16-byte aligned in global memory (up to 3 extra
+                                                // columns on the left) and rows of whole 16 bytes       (28)
 constexpr int kWinJ = kWinC + 1;                // J nodes per window edge: c .. c+1         (23)
 #ifndef GRPIC_CHUNK
 #define GRPIC_CHUNK 16384

@@ -108,11 +108,12 @@ constexpr int kTBlock = GRPIC_TILED_BLOCK;
 // ---- shared-memory layout ----
 constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
 constexpr int kNodeStride = 8;                  // reals per node: D1 D2 D3 B1 B2 B3 + 2 pad (128-bit reads)
-constexpr int kJStride = kWinF;                 // row stride of one shared J tile
+constexpr int kJStride = (kWinJ + 3) / 4 * 4;   // row stride of one shared J tile                  (24)
 constexpr int kJComp = kWinJ * kJStride;        // one component
 constexpr int kJTile = 3 * kJComp;              // one private J tile (J1 J2 J3)
 constexpr int kWarps = kTBlock / 32;
-constexpr int kRawElems = 6 * kWinF * kRowF;    // staged raw stencil; its space is reused by the J tiles after stage (i)
+constexpr int kRawComp = (kWinF * kRowF + 31) / 32 * 32;   // one staged component; TMA wants 128-byte aligned destinations
+constexpr int kRawElems = 6 * kRawComp;    // staged raw stencil; its space is reused by the J tiles after stage (i)
 constexpr int kJElems = kWarps * kJTile;        // one PRIVATE J tile per warp: no atomics inside the CTA
 constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
 constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride;
@@ -296,7 +297,7 @@ struct RawAcc {      // raw staged stencil: sample (row, col) of component c
   const T* raw;
   int row, col;
   __device__ __forceinline__ T operator()(int c, int di, int dj) const {
-    return raw[c * (kWinF * kRowF) + (row + di) * kRowF + (col + dj)];
+    return raw[c * kRawComp + (row + di) * kRowF + (col + dj)];
   }
 };
 
@@ -342,13 +343,13 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
       mbar_expect_tx(bar, 6u * kWinF * kRowF * (uint32_t)sizeof(T));
 #pragma unroll
       for (int c = 0; c < 6; ++c)
-        tma_load_2d(sF + c * kWinF * kRowF, &maps.m[c], a2lo - off2, c1lo - 1 + g.ng, bar);
+        tma_load_2d(sF + c * kRawComp, &maps.m[c], a2lo - off2, c1lo - 1 + g.ng, bar);
     }
     mbar_wait(bar, 0);
   } else {
     const int rows = g.n1 + 2 * g.ng;
     for (int e = tid; e < kRawElems; e += kTBlock) {
-      const int c = e / (kWinF * kRowF), rem = e % (kWinF * kRowF);
+      const int c = e / kRawComp, rem = e % kRawComp;
       const int a1 = c1lo - 1 + g.ng + rem / kRowF, a2 = a2lo - off2 + rem % kRowF;
       sF[e] = (a1 >= 0 && a1 < rows && a2 >= 0 && a2 < g.ld) ? __ldg(F.f[c] + (int64_t)a1 * g.ld + a2) : T(0);
     }
