@@ -1,12 +1,16 @@
 // grpic_kernels.cuh — the CUDA kernels behind include/grpic.h (sm_100a).
 //
-//   k_push          steps 1-11 + particle BCs, one thread per particle          (grpic_interp_push)
-//   k_deposit       charge-conserving deposit from (prev, current)              (grpic_deposit)
-//   k_step_direct   fused push + deposit, global gathers and global reductions  (grpic_step, unsorted)
-//   k_step_tiled    fused push + deposit over cell-sorted tiles: field stencil of the tile staged
-//                   in shared memory by TMA, J accumulated in shared memory with warp-aggregated
-//                   atomics and flushed once                                    (grpic_step, sorted)
-//   k_sort_*        counting sort by tile-major cell key + tile work-item table (grpic_sort)
+//   k_push_or_step<T,false,C>  steps 1-11 + particle BCs, one thread per particle    (grpic_interp_push, unsorted species)
+//   k_push_or_step<T,true,C>   fused push + deposit, L2 gathers and red.global.add   (grpic_step, unsorted species;
+//                              chunks of grpic_step_host; slots the tile table does not cover)
+//   k_deposit<T,C>             charge-conserving deposit from (prev, current)        (grpic_deposit, unsorted species)
+//   k_step_tiled<T,C,kDeposit> grpic_tiled.cuh: fused step over cell-sorted tiles — field stencil of the tile staged in
+//                              shared memory by TMA, J in per-warp shared tiles, one flush (grpic_step; without the
+//                              deposit half: grpic_interp_push on a sorted species)
+//   k_deposit_tiled<T,C>       grpic_tiled.cuh: the deposit half alone               (grpic_deposit, sorted species)
+//   k_sort_*, k_scan_*, k_items_*  counting sort by tile-major cell key + work-item table (grpic_sort)
+//   grpic_fields.cuh           field-solver half: auxiliary fields, Faraday, Ampere, boundary conditions, filter
+// C = coordinate class: Coord<T> (default map of the five configs, specialised) or CoordGen<T> (all maps of App. A).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>

@@ -6,7 +6,8 @@
 //      memory, completion tracked by an mbarrier; out-of-range rows/columns are zero-filled by TMA;
 //   2. stage (i) of the gather (R-S4) is done ONCE per tile: the six Yee components are averaged to the
 //      (kTile + 2 kHalo + 1)^2 nodes of the window and stored node-major (8 reals per node), so that a
-//      particle's gather is four 32/64-byte node reads and six bilinear forms;
+//      particle's gather is four 32/64-byte node reads and six bilinear forms; the columns of the next 32
+//      particles are requested before the current 32 are pushed (software pipeline);
 //   3. every thread pushes its particles (steps 1-11 + BCs); a particle that has drifted out of the
 //      window since the last sort falls back to global gathers, so the result never depends on how
 //      stale the table is;
