@@ -134,9 +134,10 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
  * is skipped and counted (n_overstep).  Errors: EINVAL, ESTATE (no push yet), ECUDA. */
 int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, void* cuda_stream);
 
-/* Fused grpic_interp_push + grpic_deposit in one kernel (previous position stays in registers but is
- * still written, so that grpic_deposit / diagnostics see it).  Same results as the two calls up to
- * the order of the J additions.  J may be NULL iff charge == 0. */
+/* Fused grpic_interp_push + grpic_deposit in one kernel: the previous position (step 1) stays
+ * in registers.  It is also written to the four *_prev columns when they are given (so that a later
+ * grpic_deposit / diagnostics see it); all four may be NULL, and then it is not stored at all.  Same
+ * results as the two calls up to the order of the J additions.  J may be NULL iff charge == 0. */
 int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, grpic_current* J,
                double dt, void* cuda_stream);
 
@@ -147,6 +148,14 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
  * shared-memory path uses for this species (keyed by the address of p->i1).
  * Errors: EINVAL, ENOMEM, ECUDA. */
 int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* cuda_stream);
+
+/* The same sort out of place: reads the columns of `src` (left unchanged) and writes them in sorted order
+ * into the columns of `dst` — same n, same optional columns, no column shared between the two.  Saves the
+ * library-side snapshot of every column that the in-place call needs (a caller that keeps two column sets
+ * and swaps them after each sort moves every byte once instead of twice).  The tile table is built for
+ * `dst` (keyed by the address of dst->i1).  In both calls phi and the four *_prev columns are optional
+ * (*_prev: all or none).  Errors: EINVAL, ENOMEM, ECUDA. */
+int grpic_sort_into(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* dst, void* cuda_stream);
 int grpic_tile_size(void);
 
 /* Compaction / injection support.  After grpic_sort the alive particles of the species occupy the slots

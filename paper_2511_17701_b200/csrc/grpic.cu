@@ -117,15 +117,18 @@ PPtrs<real> make_pptrs(const grpic_particles* p) {
   return P;
 }
 
-int check_particles(grpic_ctx* ctx, const grpic_particles* p, bool need_prev) {
+// need_prev: 0 = the *_prev columns are not looked at, 1 = required, 2 = all four or none
+int check_particles(grpic_ctx* ctx, const grpic_particles* p, int need_prev) {
   if (!p) return fail(ctx, GRPIC_EINVAL, "particles == NULL");
   if (p->n < 0) return fail(ctx, GRPIC_EINVAL, "particles.n < 0");
   if (p->n > 0xfffffff0ll) return fail(ctx, GRPIC_EINVAL, "particles.n exceeds 2^32 - 16");
   if (p->n == 0) return GRPIC_OK;
   if (!p->i1 || !p->i2 || !p->dx1 || !p->dx2 || !p->u1 || !p->u2 || !p->u3 || !p->weight || !p->tag)
     return fail(ctx, GRPIC_EINVAL, "a required particle column is NULL");
-  if (need_prev && (!p->i1_prev || !p->i2_prev || !p->dx1_prev || !p->dx2_prev))
-    return fail(ctx, GRPIC_EINVAL, "a *_prev particle column is NULL");
+  const int n_prev = (p->i1_prev != nullptr) + (p->i2_prev != nullptr) + (p->dx1_prev != nullptr) + (p->dx2_prev != nullptr);
+  if (need_prev == 1 && n_prev != 4) return fail(ctx, GRPIC_EINVAL, "a *_prev particle column is NULL");
+  if (need_prev == 2 && n_prev != 4 && n_prev != 0)
+    return fail(ctx, GRPIC_EINVAL, "the *_prev particle columns must be all present or all NULL");
   return GRPIC_OK;
 }
 
@@ -328,7 +331,7 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
 
 int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, p, true);
+  int rc = check_particles(ctx, p, 1);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
   const SpeciesConst sc = make_species(p, dt, false);
@@ -368,7 +371,7 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
 
 int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, p, true);
+  int rc = check_particles(ctx, p, 1);
   if (rc) return rc;
   if (!ctx->have_dt) return fail(ctx, GRPIC_ESTATE, "grpic_deposit before any grpic_interp_push on this context");
   const SpeciesConst sc = make_species(p, ctx->last_dt, true);
@@ -401,7 +404,7 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
 int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, grpic_current* J, double dt,
                void* stream) {
   if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, p, true);
+  int rc = check_particles(ctx, p, 2);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
   const SpeciesConst sc = make_species(p, dt, true);
@@ -438,20 +441,23 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   return GRPIC_OK;
 }
 
-int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
-  if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, p, true);
-  if (rc) return rc;
-  cudaStream_t st = (cudaStream_t)stream;
+namespace {
+// Counting sort of the columns of `src` into the columns of `p`.  src == p: in place from the caller's view
+// (every column is first copied to library scratch); src != p: the gather reads the caller's source columns
+// directly, no snapshot.  The *_prev columns and phi are optional (same set on both sides).
+int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cudaStream_t st) {
+  int rc;
   const int64_t n = p->n;
   if (n == 0) return GRPIC_OK;
+  const bool in_place = (src == p);
+  const bool has_prev = src->i1_prev != nullptr;
   const SortGeom sg = sort_geom(ctx);
   const uint32_t n_tiles = (uint32_t)sg.nt1 * sg.nt2;
   // scratch (grown on demand; growing synchronises)
   const size_t col = ((size_t)n * sizeof(real) + 255) / 256 * 256;
   const size_t col4 = ((size_t)n * 4 + 255) / 256 * 256;
   const size_t col1 = ((size_t)n + 255) / 256 * 256;
-  const size_t need = 9 * col + 4 * col4 + col1;
+  const size_t need = in_place ? 9 * col + 4 * col4 + col1 : 256;
   if (ctx->cap_particles < n) {
     CK(cudaStreamSynchronize(st));
     cudaFree(ctx->d_keys); cudaFree(ctx->d_dest);
@@ -482,7 +488,7 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
   }
   // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks (inverse permutation); 4. snapshot; 5. gather
   CK(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)sg.n_keys + 1) * 4, st));
-  k_sort_hist<<<grid_for(n), kBlock, 0, st>>>(sg, n, p->i1, p->i2, p->tag, ctx->d_keys, ctx->d_hist);
+  k_sort_hist<<<grid_for(n), kBlock, 0, st>>>(sg, n, src->i1, src->i2, src->tag, ctx->d_keys, ctx->d_hist);
   if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
 
   // tile table from the offsets (before the cursor copy is consumed)
@@ -507,34 +513,37 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
 
   k_sort_rank<<<grid_for(n), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
 
-  // snapshot of every column in library scratch (plain contiguous copies), then ONE gather back into the
-  // caller's columns in sorted order
-  char* s = (char*)ctx->d_scratch;
-  PPtrs<real> out = make_pptrs(p), in;
-  in.n = n;
-  in.dx1 = (real*)s; s += col; in.dx2 = (real*)s; s += col;
-  in.u1 = (real*)s; s += col; in.u2 = (real*)s; s += col; in.u3 = (real*)s; s += col;
-  in.phi = p->phi ? (real*)s : nullptr; s += col;
-  in.dx1p = (real*)s; s += col; in.dx2p = (real*)s; s += col;
-  in.w = (const real*)s; s += col;
-  in.i1 = (int32_t*)s; s += col4; in.i2 = (int32_t*)s; s += col4;
-  in.i1p = (int32_t*)s; s += col4; in.i2p = (int32_t*)s; s += col4;
-  in.tag = (uint8_t*)s;
-  const size_t rb = (size_t)n * sizeof(real), ib = (size_t)n * 4;
-  CK(cudaMemcpyAsync(in.dx1, p->dx1, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.dx2, p->dx2, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.u1, p->u1, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.u2, p->u2, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.u3, p->u3, rb, cudaMemcpyDeviceToDevice, st));
-  if (p->phi) CK(cudaMemcpyAsync(in.phi, p->phi, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.dx1p, p->dx1_prev, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.dx2p, p->dx2_prev, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync((void*)in.w, p->weight, rb, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.i1, p->i1, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.i2, p->i2, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.i1p, p->i1_prev, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.i2p, p->i2_prev, ib, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemcpyAsync(in.tag, p->tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
+  // in place: snapshot of every column in library scratch (plain contiguous copies); then ONE gather into the
+  // destination columns in sorted order
+  PPtrs<real> out = make_pptrs(p), in = make_pptrs(src);
+  if (in_place) {
+    char* s = (char*)ctx->d_scratch;
+    in.dx1 = (real*)s; s += col; in.dx2 = (real*)s; s += col;
+    in.u1 = (real*)s; s += col; in.u2 = (real*)s; s += col; in.u3 = (real*)s; s += col;
+    in.phi = p->phi ? (real*)s : nullptr; s += col;
+    in.dx1p = has_prev ? (real*)s : nullptr; s += col; in.dx2p = has_prev ? (real*)s : nullptr; s += col;
+    in.w = (const real*)s; s += col;
+    in.i1 = (int32_t*)s; s += col4; in.i2 = (int32_t*)s; s += col4;
+    in.i1p = has_prev ? (int32_t*)s : nullptr; s += col4; in.i2p = has_prev ? (int32_t*)s : nullptr; s += col4;
+    in.tag = (uint8_t*)s;
+    const size_t rb = (size_t)n * sizeof(real), ib = (size_t)n * 4;
+    CK(cudaMemcpyAsync(in.dx1, p->dx1, rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.dx2, p->dx2, rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.u1, p->u1, rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.u2, p->u2, rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.u3, p->u3, rb, cudaMemcpyDeviceToDevice, st));
+    if (p->phi) CK(cudaMemcpyAsync(in.phi, p->phi, rb, cudaMemcpyDeviceToDevice, st));
+    if (has_prev) {
+      CK(cudaMemcpyAsync(in.dx1p, p->dx1_prev, rb, cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(in.dx2p, p->dx2_prev, rb, cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(in.i1p, p->i1_prev, ib, cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(in.i2p, p->i2_prev, ib, cudaMemcpyDeviceToDevice, st));
+    }
+    CK(cudaMemcpyAsync((void*)in.w, p->weight, rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.i1, p->i1, ib, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.i2, p->i2, ib, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(in.tag, p->tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
+  }
   k_sort_gather<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
   CK(cudaGetLastError());
   // number of alive particles (they now occupy [0, n_alive)): 4 bytes read back, the one synchronisation of the sort
@@ -543,6 +552,33 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
   CK(cudaStreamSynchronize(st));
   ss.n_alive = (int64_t)h_alive;
   return GRPIC_OK;
+}
+}  // namespace
+
+int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, p, 2);
+  if (rc) return rc;
+  return sort_impl(ctx, p, p, (cudaStream_t)stream);
+}
+
+int grpic_sort_into(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* dst, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  int rc = check_particles(ctx, src, 2);
+  if (rc || (rc = check_particles(ctx, dst, 2))) return rc;
+  if (src->n != dst->n) return fail(ctx, GRPIC_EINVAL, "sort_into: src.n != dst.n");
+  if (src->n == 0) return GRPIC_OK;
+  if ((src->phi != nullptr) != (dst->phi != nullptr) || (src->i1_prev != nullptr) != (dst->i1_prev != nullptr))
+    return fail(ctx, GRPIC_EINVAL, "sort_into: src and dst must carry the same optional columns");
+  // no column of dst may be a column of src (the gather reads src while dst is written)
+  const void* a[14] = {src->i1, src->i2, src->dx1, src->dx2, src->u1, src->u2, src->u3, src->phi, src->i1_prev,
+                       src->i2_prev, src->dx1_prev, src->dx2_prev, src->weight, src->tag};
+  const void* b[14] = {dst->i1, dst->i2, dst->dx1, dst->dx2, dst->u1, dst->u2, dst->u3, dst->phi, dst->i1_prev,
+                       dst->i2_prev, dst->dx1_prev, dst->dx2_prev, dst->weight, dst->tag};
+  for (int i = 0; i < 14; ++i)
+    for (int j = 0; j < 14; ++j)
+      if (a[i] && a[i] == b[j]) return fail(ctx, GRPIC_EINVAL, "sort_into: src and dst share a column");
+  return sort_impl(ctx, src, dst, (cudaStream_t)stream);
 }
 
 int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_alive) {
@@ -772,7 +808,7 @@ int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3*
 int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh, grpic_current* Jh, double dt,
                     int64_t* h2d_bytes, int64_t* d2h_bytes) {
   if (!ctx) return GRPIC_EINVAL;
-  int rc = check_particles(ctx, ph, false);
+  int rc = check_particles(ctx, ph, 0);
   if (rc) return rc;
   const bool want_prev = ph->i1_prev && ph->i2_prev && ph->dx1_prev && ph->dx2_prev;   // all four or none come back
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
@@ -841,8 +877,8 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
     P.dx1 = (real*)base[2]; P.dx2 = (real*)base[3];
     P.u1 = (real*)base[4]; P.u2 = (real*)base[5]; P.u3 = (real*)base[6];
     P.phi = ph->phi ? (real*)base[7] : nullptr;
-    P.i1p = (int32_t*)base[8]; P.i2p = (int32_t*)base[9];
-    P.dx1p = (real*)base[10]; P.dx2p = (real*)base[11];
+    P.i1p = want_prev ? (int32_t*)base[8] : nullptr; P.i2p = want_prev ? (int32_t*)base[9] : nullptr;
+    P.dx1p = want_prev ? (real*)base[10] : nullptr; P.dx2p = want_prev ? (real*)base[11] : nullptr;
     P.w = (const real*)base[12]; P.tag = (uint8_t*)base[13];
     const size_t rb = (size_t)m * sizeof(real), ib = (size_t)m * 4;
 #define UP(dst, src, bytes) do { CK(cudaMemcpyAsync((void*)(dst), (src) + lo, bytes, cudaMemcpyHostToDevice, st)); up += (int64_t)(bytes); } while (0)

@@ -114,7 +114,7 @@ __device__ __forceinline__ void particle_direct(const Consts<T>& g, const PPtrs<
     const int ia = p.i1, ja = p.i2;
     const T xa = p.dx1, ya = p.dx2;
     // step 1
-    P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya;
+    if (!kDeposit || P.i1p) { P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya; }   // optional for the fused step
     T Dp[3] = {T(0), T(0), T(0)}, Bp[3] = {T(0), T(0), T(0)};
     const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
     if (sc.em) {
@@ -253,8 +253,10 @@ __global__ void __launch_bounds__(kBlock) k_sort_gather(const PPtrs<T> in, const
   out.dx1[d] = in.dx1[k]; out.dx2[d] = in.dx2[k];
   out.u1[d] = in.u1[k]; out.u2[d] = in.u2[k]; out.u3[d] = in.u3[k];
   if (in.phi) out.phi[d] = in.phi[k];
-  out.i1p[d] = in.i1p[k]; out.i2p[d] = in.i2p[k];
-  out.dx1p[d] = in.dx1p[k]; out.dx2p[d] = in.dx2p[k];
+  if (in.i1p) {
+    out.i1p[d] = in.i1p[k]; out.i2p[d] = in.i2p[k];
+    out.dx1p[d] = in.dx1p[k]; out.dx2p[d] = in.dx2p[k];
+  }
   const_cast<T*>(out.w)[d] = in.w[k];
   out.tag[d] = in.tag[k];
 }

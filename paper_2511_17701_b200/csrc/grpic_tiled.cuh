@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
     if (alive) {
       const int ia = p.i1, ja = p.i2;
       const T xa = p.dx1, ya = p.dx2;
-      P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya;
+      if (!kDeposit || P.i1p) { P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya; }
       const int wa1 = ia - c1lo, wa2 = ja - c2lo;                       // cell inside the window?
       const bool a_in = (unsigned)wa1 < (unsigned)kWinC && (unsigned)wa2 < (unsigned)kWinC;
       const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);

@@ -23,7 +23,7 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
-           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current"]
+           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into"]
 
 
 class GrpicError(RuntimeError):
@@ -87,6 +87,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_deposit.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Current), _vp]
     lib.grpic_step.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Fields), C.POINTER(_Current), C.c_double, _vp]
     lib.grpic_sort.argtypes = [_vp, C.POINTER(_Particles), _vp]
+    lib.grpic_sort_into.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Particles), _vp]
     lib.grpic_counters.argtypes = [_vp] + [C.POINTER(C.c_int64)] * 4 + [_vp]
     lib.grpic_updates_total.argtypes = [_vp, C.POINTER(C.c_int64), _vp]
     lib.grpic_step_host.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Fields), C.POINTER(_Current), C.c_double,
@@ -161,6 +162,18 @@ class ParticleSet:
             src = getattr(sp, k, None)
             cols[k] = put(src if src is not None else np.zeros(n, dt), dt)
         return cls(cols, sp.q_over_m, sp.charge, sp.massive)
+
+    def drop_prev(self):
+        """forget the four *_prev columns (the fused step and the sort do without them)"""
+        for k in ("i1_prev", "i2_prev", "dx1_prev", "dx2_prev"):
+            self.cols[k] = None
+        return self
+
+    def empty_like(self):
+        """a second column set of the same shape (uninitialised): the other half of a sort_into ping-pong"""
+        torch = _torch()
+        return ParticleSet({k: (None if v is None else torch.empty_like(v)) for k, v in self.cols.items()},
+                           self.q_over_m, self.charge, self.massive)
 
     def clone(self):
         return ParticleSet({k: (None if v is None else v.clone()) for k, v in self.cols.items()},
@@ -277,6 +290,11 @@ class Context:
     def sort(self, p: ParticleSet, stream=None):
         ps = p.c_struct()
         self._ck(self.lib.grpic_sort(self.h, C.byref(ps), _stream_ptr(stream)))
+
+    def sort_into(self, src: ParticleSet, dst: ParticleSet, stream=None):
+        """out-of-place sort: src -> dst (two column sets that the caller swaps), no snapshot inside"""
+        a = src.c_struct(); b = dst.c_struct()
+        self._ck(self.lib.grpic_sort_into(self.h, C.byref(a), C.byref(b), _stream_ptr(stream)))
 
     def sorted_alive(self, p: ParticleSet) -> int:
         """alive particles of the species at its last sort; they occupy the slots [0, n_alive)"""

@@ -96,6 +96,10 @@ TOL = {"f64": dict(x=1e-12, u=1e-12, J=1e-10), "f32": dict(x=1e-5, u=1e-5, J=1e-
 def oracle_from_cols(O, cols, q_over_m, charge, massive):
     """numpy column dict (ParticleSet.to_numpy()) -> oracle Particles (FP64 copies of the same values)."""
     f = lambda k: np.asarray(cols[k], np.float64)
+    if cols.get("i1_prev") is None:          # species kept without *_prev columns (fused step only)
+        n = len(cols["i1"])
+        cols = dict(cols, i1_prev=np.zeros(n, np.int32), i2_prev=np.zeros(n, np.int32),
+                    dx1_prev=np.zeros(n), dx2_prev=np.zeros(n))
     return O.Particles(i1=cols["i1"], i2=cols["i2"], dx1=f("dx1"), dx2=f("dx2"), u1=f("u1"), u2=f("u2"), u3=f("u3"),
                        weight=f("weight"), tag=cols["tag"], phi=None if cols.get("phi") is None else f("phi"),
                        i1_prev=cols["i1_prev"], i2_prev=cols["i2_prev"], dx1_prev=f("dx1_prev"),

@@ -61,7 +61,8 @@ def _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode, sort_first=F
     alive, a_in, a_out = O.push(g, op, fhost if ps.q_over_m != 0 and ps.massive else None, dt, diag=diag)
     Jo, over = O.deposit(g, op, dt)
     after = ps.to_numpy()
-    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag)
+    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag,
+                            check_prev=before["i1_prev"] is not None)
     if res["n_idx_mismatch"] == 0:
         assert (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"]) == (alive, a_in, a_out, over), (c, alive, a_in, a_out, over)
         res.update(compare_current(Jo, _J_np(J), prec))
@@ -264,6 +265,71 @@ def test_sort_is_a_permutation_into_key_order(G, O, W):
     assert np.all(after["tag"][: int((before["tag"] != 0).sum())] == 1)       # dead at the tail
     ref, _, key_ref = O.sort_reference(g, oracle_from_cols(O, before, -1.0, -1.0, 1), T)
     assert np.array_equal(key, key_ref)
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_sort_into_and_species_without_prev_columns(G, O, W, prec):
+    """grpic_sort_into (two column sets, no snapshot) and the optional *_prev columns: the destination is the
+    source permuted into key order, the source is untouched, and the fused tile-path step on the destination
+    agrees with the oracle; several sort/step rounds swapping the two sets."""
+    wl = W.config_magnetosphere(shrink=8)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    fdev, fhost = _fields_both(G, wl, prec)
+    sp = wl.species[0]
+    rng = np.random.default_rng(11)
+    perm = rng.permutation(sp.n)
+    for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "weight", "tag", "phi"):
+        setattr(sp, k, getattr(sp, k)[perm])
+    sp.tag = sp.tag.copy(); sp.tag[rng.random(sp.n) < 0.05] = 0
+    assert sp.n < (1 << 24)
+    sp.phi = np.arange(sp.n, dtype=np.float64)                                # unique id (exact in FP32)
+    a = G.ParticleSet.from_host(sp, prec).drop_prev()
+    b = a.empty_like()
+    T = ctx.tile_size()
+    before = a.to_numpy()
+    ctx.sort_into(a, b)
+    src_after, dst = a.to_numpy(), b.to_numpy()
+    ids = dst["phi"].astype(np.int64)
+    assert np.array_equal(np.sort(ids), np.arange(sp.n))
+    for k, v in dst.items():
+        if v is not None:
+            assert np.array_equal(src_after[k], before[k]), k                 # source untouched
+            assert np.array_equal(v, before[k][ids]), k                       # every column moved alike
+        else:
+            assert k.endswith("_prev")
+    key, _ = O.sort_key(g, dst["i1"], dst["i2"], dst["tag"], T)
+    _, _, key_ref = O.sort_reference(g, oracle_from_cols(O, before, -1.0, -1.0, 1), T)
+    assert np.array_equal(key, key_ref)
+    assert ctx.sorted_alive(b) == int((before["tag"] != 0).sum())
+    # sort / step rounds, swapping the two sets; every step against the oracle
+    cur, other = b, a
+    for rnd in range(3):
+        for _ in range(2):
+            res, c = _one_step_parity(G, O, ctx, g, cur, fdev, fhost, wl.dt, prec, "fused")
+        ctx.sort_into(cur, other)
+        cur, other = other, cur
+        cols = cur.to_numpy()
+        key, _ = O.sort_key(g, cols["i1"], cols["i2"], cols["tag"], T)
+        assert np.all(np.diff(key) >= 0)
+    # the in-place sort takes a species without *_prev columns too
+    ctx.sort(cur)
+    res, c = _one_step_parity(G, O, ctx, g, cur, fdev, fhost, wl.dt, prec, "fused")
+    # refused: a shared column, a partial set of *_prev columns, different optional columns
+    bad = cur.empty_like(); bad.cols["u1"] = cur.cols["u1"]
+    with pytest.raises(G.GrpicError):
+        ctx.sort_into(cur, bad)
+    import torch
+    part = cur.empty_like(); part.cols["i1_prev"] = torch.zeros_like(part.cols["i1"])
+    with pytest.raises(G.GrpicError):
+        ctx.sort(part)
+    with pytest.raises(G.GrpicError):
+        ctx.step(part, fdev, _zeros_J(G, ctx, prec), wl.dt)
+    full = G.ParticleSet.from_host(sp, prec)
+    with pytest.raises(G.GrpicError):
+        ctx.sort_into(cur, full)
+    with pytest.raises(G.GrpicError):                                         # the split calls still need them
+        ctx.interp_push(cur, fdev, wl.dt)
 
 
 def test_step_host_matches_device_step(G, O, W):
