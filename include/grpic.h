@@ -107,7 +107,8 @@ int grpic_destroy(grpic_ctx* ctx);
  * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernel after a grpic_sort;
  *              0 forces the direct kernel (global gathers and atomics).
  * "tma": 1 (default) stages the tile's field stencil with TMA; 0 uses plain cooperative loads (also the
- *        automatic choice when a field array is not 16-byte aligned or (n2 + 2 nghost)*sizeof(real) % 16 != 0). */
+ *        automatic choice when a field array is not 16-byte aligned or (n2 + 2 nghost)*sizeof(real) % 16 != 0).
+ * "host_chunk": particles per chunk of grpic_step_host, 2^10..2^26 (default 2^22; three chunks in flight). */
 int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t value);
 /* "small_angle": theta used in any metric evaluation is clamped to [eps, pi - eps] (R-S9).
  * "r0", "h0":    the remaining parameters of the quasi-spherical map of App. A.3, both 0 by default:
@@ -225,8 +226,9 @@ int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3*
 
 /* End-to-end convenience: every pointer in p, fields and J is HOST memory (pinned or pageable).
  * Copies fields and particle columns to library-owned device buffers in chunks, runs the fused step
- * chunk by chunk (copies overlapped with compute on two streams), accumulates J on the device and
- * copies the particle columns and J back; J_host += .  The four *_prev columns of p_host may all be NULL:
+ * chunk by chunk (three chunks in flight on three streams: upload, compute, download), and copies the
+ * particle columns back; J_host += (the host values are uploaded, the deposit adds to them on the device, the
+ * sums come back).  The four *_prev columns of p_host may all be NULL:
  * the fused step keeps the previous position on the device and nothing is copied back for them.
  * Synchronous.  Bytes moved are reported through
  * h2d_bytes / d2h_bytes (may be NULL).  Errors as grpic_step, plus ENOMEM. */

@@ -41,6 +41,7 @@ struct grpic_ctx {
   grpic_grid grid;
   double a, r_min, r_max, small_angle, r0, h0, mass, k_J;
   int n_iter, tile_path, use_tma, early_exit;
+  int64_t host_chunk;       // particles per chunk of grpic_step_host
   double last_dt;
   bool have_dt;
   unsigned long long* d_counters;   // 5: four of the last call + cumulative updates
@@ -239,6 +240,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->k_J = 4.0 * M_PI;                                    // coefficient of J in Ampere's law (Eq. 37)
   ctx->n_iter = 10;
   ctx->tile_path = 1;
+  ctx->host_chunk = 1 << 22;
   ctx->use_tma = 1;
   ctx->early_exit = 1;
   ctx->have_dt = false; ctx->last_dt = 0.0;
@@ -295,6 +297,11 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t v) {
   }
   if (!std::strcmp(key, "tma")) {
     ctx->use_tma = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "host_chunk")) {
+    if (v < 1024 || v > (1 << 26)) return fail(ctx, GRPIC_EINVAL, "host_chunk must be in 2^10..2^26");
+    ctx->host_chunk = v;
     return GRPIC_OK;
   }
   return fail(ctx, GRPIC_EINVAL, std::string("unknown integer key: ") + key);
@@ -832,7 +839,9 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
     }
     ctx->h_fields_bytes = 9 * gbytes;
   }
-  const int64_t chunk = 1 << 22;                       // particles per chunk
+  // particles per chunk: three chunks in flight.  Measured on config 4 (ms per step, both species): 2^22 117.5,
+  // 2^21 118.6, 2^20 125.5, 2^18 170 - below 4 MB per column copy the per-copy cost of the engines shows
+  const int64_t chunk = ctx->host_chunk;
   const size_t cb = (size_t)chunk * 8;                 // widest column
   if (ctx->h_cap < cb) {
     for (auto& q : ctx->h_dev) { cudaFree(q); q = nullptr; }
@@ -858,16 +867,36 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
   }
   JPtrs<real> Jp{{nullptr, nullptr, nullptr}};
   if (sc.do_deposit) {
-    CK(cudaMemsetAsync(dgrid + 6 * cells, 0, 3 * gbytes, s0));
-    for (int k = 0; k < 3; ++k) Jp.j[k] = dgrid + (6 + k) * cells;
+    // J_host += : the host values go up, the deposit adds on the device, the sums come back
+    real* src[3] = {Jh->J1, Jh->J2, Jh->J3};
+    for (int k = 0; k < 3; ++k) {
+      Jp.j[k] = dgrid + (6 + k) * cells;
+      CK(cudaMemcpyAsync(Jp.j[k], src[k], gbytes, cudaMemcpyHostToDevice, s0));
+      up += (int64_t)gbytes;
+    }
   }
   CK(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), s0));
   CK(cudaStreamSynchronize(s0));
   ctx->last_dt = dt; ctx->have_dt = true;
   const Consts<real> g = make_consts(ctx);
+  // chunk sizes: the first upload and the last download of a call overlap nothing, so a long call ramps up
+  // (chunk/8, /4, /2), runs full chunks, and ramps down again
+  std::vector<int64_t> sizes;
+  {
+    int64_t body = ph->n;
+    const int64_t ramp[3] = {chunk / 8, chunk / 4, chunk / 2};
+    const bool ramped = ph->n >= 4 * chunk && chunk >= 8192;
+    if (ramped) {
+      for (int k = 0; k < 3; ++k) { sizes.push_back(ramp[k]); body -= 2 * ramp[k]; }
+    }
+    for (; body > 0; body -= chunk) sizes.push_back(body < chunk ? body : chunk);
+    if (ramped)
+      for (int k = 2; k >= 0; --k) sizes.push_back(ramp[k]);
+  }
   int buf = 0;
-  for (int64_t lo = 0; lo < ph->n; lo += chunk, buf = (buf + 1) % 3) {
-    const int64_t m = (ph->n - lo < chunk) ? ph->n - lo : chunk;
+  int64_t lo = 0;
+  for (size_t ci = 0; ci < sizes.size(); lo += sizes[ci], ++ci, buf = (buf + 1) % 3) {
+    const int64_t m = sizes[ci];
     cudaStream_t st = ctx->h_streams[buf];
     char* base[16];
     for (int k = 0; k < 16; ++k) base[k] = (char*)ctx->h_dev[k] + (size_t)buf * cb;
@@ -907,14 +936,12 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh,
   }
   for (auto& q : ctx->h_streams) CK(cudaStreamSynchronize(q));
   if (sc.do_deposit) {
-    std::vector<real> tmp;
-    try { tmp.resize(cells); } catch (...) { return fail(ctx, GRPIC_ENOMEM, "host staging allocation failed"); }
     real* dst[3] = {Jh->J1, Jh->J2, Jh->J3};
     for (int k = 0; k < 3; ++k) {
-      CK(cudaMemcpy(tmp.data(), dgrid + (6 + k) * cells, gbytes, cudaMemcpyDeviceToHost));
+      CK(cudaMemcpyAsync(dst[k], Jp.j[k], gbytes, cudaMemcpyDeviceToHost, s0));
       down += (int64_t)gbytes;
-      for (size_t c = 0; c < cells; ++c) dst[k][c] += tmp[c];
     }
+    CK(cudaStreamSynchronize(s0));
   }
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = down;

@@ -367,6 +367,20 @@ def test_step_host_matches_device_step(G, O, W):
     assert np.all(c2["i1_prev"] == -7) and np.all(c2["i2_prev"] == -7)
     for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "phi", "tag"):
         assert np.array_equal(a[k], c2[k]), k
+    # many chunks with the ramped sizes at both ends of the call, and J_host += on top of what is there
+    assert sp.n >= 4 * 8192
+    ctx.set_int("host_chunk", 8192)
+    ph3 = G.ParticleSet.from_host(sp, "f32", device="cpu", pinned=True)
+    up3, down3 = ctx.step_host(ph3, fhost, Jh2, wl.dt)
+    c3 = ph3.to_numpy()
+    for k in a:
+        if a[k] is not None:
+            assert np.array_equal(a[k], c3[k]), k
+    for k in Jd:
+        assert torch.allclose(2 * Jd[k].cpu(), Jh2[k], rtol=0, atol=2e-5 * float(Jd[k].abs().max()))
+    assert ctx.counters() == cd
+    with pytest.raises(G.GrpicError):
+        ctx.set_int("host_chunk", 7)
 
 
 def test_edge_cases(G, O, W):
