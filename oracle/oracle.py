@@ -399,6 +399,47 @@ def field_bc(g: Grid, fields: dict, n_const: int = -1) -> dict:
 
 
 # ----------------------------------------------------------------------------------------------
+# Absorbing layer at the outer radial boundary ("the fields are matched to their initial values using an
+# absorbing layer"; "In the absorbing layer, we smoothly match the field components with the analytic
+# solution").  The paper defers the profile to paper I.  Reading R-F6 of DESIGN.md: in the layer r_abs < r the field
+# relaxes toward the target with the weight
+#     s(r) = tanh(4 (r_max - r) / (r_max - r_abs)),   F <- F_target + s (F - F_target),
+# every component at its own Yee radius (D^1, B^2, B^3 at i+1/2; D^2, D^3, B^1 at i); rows beyond r_max take the
+# target; rows with r <= r_abs are not touched.  The PROFILE is parity unpinned (paper I); the pins check what any
+# such layer must do: a fixed point at the target, untouched interior, monotone weight, and that an outgoing pulse
+# is absorbed instead of reflected.
+# ----------------------------------------------------------------------------------------------
+_X1_OFFSET = {"D1": 0.5, "D2": 0.0, "D3": 0.0, "B1": 0.0, "B2": 0.5, "B3": 0.5}
+
+
+def radius(g: Grid, x1):
+    """r(x1) of the radial map (App. A.2 / A.3)"""
+    x1 = np.asarray(x1, np.float64)
+    if g.linear_r:
+        return g.r_min + x1 * ((g.r_max - g.r_min) / g.n1)
+    lo = np.log(g.r_min - g.r0)
+    return g.r0 + np.exp(lo + x1 * ((np.log(g.r_max - g.r0) - lo) / g.n1))
+
+
+def match_weight(g: Grid, r, r_abs: float):
+    r = np.asarray(r, np.float64)
+    d = np.clip((g.r_max - r) / (g.r_max - r_abs), 0.0, None)
+    return np.tanh(4.0 * d)
+
+
+def field_match(g: Grid, fields: dict, target: dict, r_abs: float) -> dict:
+    """In place on dict(D1..B3) of float64 arrays [n1+2ng][n2+2ng]; target: the same keys (initial / analytic fields)."""
+    G = g.ng
+    for k, off in _X1_OFFSET.items():
+        r = radius(g, np.arange(-G, g.n1 + G, dtype=np.float64) + off)
+        rows = np.nonzero(r > r_abs)[0]
+        s = match_weight(g, r[rows], r_abs)[:, None]
+        A, T = fields[k], np.asarray(target[k], np.float64)
+        A[rows, :] = T[rows, :] + s * (A[rows, :] - T[rows, :])
+    return fields
+
+
+# ----------------------------------------------------------------------------------------------
 # Current filter (P:338, P:467: "n_f passes of a digital filter", details deferred to paper I).  Reading R-F5: the
 # standard binomial 1-2-1 smoothing of PIC codes, separable in x1 and x2, one pass = [1 2 1]/4 along each axis, on
 # each component's own Yee lattice; beyond the polar axes the neighbour is the mirror sample with the component's

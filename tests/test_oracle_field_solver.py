@@ -227,3 +227,73 @@ def test_current_filter_properties(O):
     O.filter_current(g, J2, 1)
     lhs = J1["J1"][3:-2, G:G + g.n2 + 1] - J1["J1"][2:-3, G:G + g.n2 + 1]
     assert np.allclose(lhs, J2["J1"][3:-2, G:G + g.n2 + 1], atol=1e-13)
+
+
+def test_absorbing_layer_fixed_point_edges_and_weight(O):
+    """Reading R-F6: what any matching layer must do, whatever its profile - fields equal to the target
+    are a fixed point (bit for bit), rows at r <= r_abs are untouched, rows beyond r_max take the target, the weight
+    falls monotonically from ~1 at r_abs to 0 at r_max, and every component uses its own Yee radius."""
+    for kw in (dict(), dict(linear_r=1), dict(r0=0.4)):
+        g = O.Grid(40, 8, 0.8, 1.5, 12.0, **kw)
+        G = g.ng
+        rng = np.random.default_rng(3)
+        keys = ("D1", "D2", "D3", "B1", "B2", "B3")
+        tgt = {k: rng.normal(size=g.shape) for k in keys}
+        f = {k: v.copy() for k, v in tgt.items()}
+        O.field_match(g, f, tgt, 9.0)
+        for k in keys:
+            assert np.array_equal(f[k], tgt[k])
+        f = {k: rng.normal(size=g.shape) for k in keys}
+        f0 = {k: v.copy() for k, v in f.items()}
+        O.field_match(g, f, tgt, 9.0)
+        assert np.isclose(O.radius(g, 0.0), g.r_min) and np.isclose(O.radius(g, float(g.n1)), g.r_max)
+        for k in keys:
+            off = 0.5 if k in ("D1", "B2", "B3") else 0.0
+            r = O.radius(g, np.arange(-G, g.n1 + G) + off)
+            inner, outer = r <= 9.0, r >= g.r_max
+            assert inner.sum() > 10 and (~inner & ~outer).sum() >= 2
+            assert np.array_equal(f[k][inner], f0[k][inner])
+            assert np.array_equal(f[k][outer], tgt[k][outer])
+            lay = ~inner & ~outer
+            s = (f[k][lay] - tgt[k][lay]) / (f0[k][lay] - tgt[k][lay])              # the weight actually applied
+            assert np.allclose(s, s[:, :1], rtol=1e-9)                                # a function of r only
+            assert np.all(np.diff(s[:, 0]) < 0) and 0.0 < s[-1, 0] and s[0, 0] < 1.0
+            assert np.allclose(s[:, 0], np.tanh(4 * (g.r_max - r[lay]) / (g.r_max - 9.0)), rtol=1e-9)
+        # staggered components see a different radius than the node-centred ones in the same row
+        row = np.nonzero((O.radius(g, np.arange(-G, g.n1 + G) + 0.0) > 9.0))[0][2]
+        s_node = (f["D2"][row, 3] - tgt["D2"][row, 3]) / (f0["D2"][row, 3] - tgt["D2"][row, 3])
+        s_half = (f["D1"][row, 3] - tgt["D1"][row, 3]) / (f0["D1"][row, 3] - tgt["D1"][row, 3])
+        assert s_half < s_node
+    w = O.match_weight(g, np.array([9.0, 10.5, 12.0, 13.0]), 9.0)
+    assert np.allclose(w, [np.tanh(4.0), np.tanh(2.0), 0.0, 0.0])
+
+
+def test_absorbing_layer_absorbs_an_outgoing_pulse(O):
+    """Flat space (App. A.1), vacuum, a toroidal Gaussian pulse of B^3 at r = 6 on r in [2, 12]: it splits into an
+    ingoing and an outgoing half; after both have reached the outer edge (t = 26), the interior r < 10 still holds
+    an O(1) field when the boundary rows are simply held (reflection), and < 2 % of the initial amplitude with the
+    layer over r in [10, 12] matching to the zero target.  A layer whose weight ran the wrong way (0 at its
+    inner edge) reflects at r_abs and fails the second bound."""
+    def run(layer):
+        g = O.Grid(160, 8, 0.0, 2.0, 12.0, linear_r=1, mass=0.0)
+        G = g.ng
+        keys = ("D1", "D2", "D3", "B1", "B2", "B3")
+        f = {k: np.zeros(g.shape) for k in keys}
+        tgt = {k: np.zeros(g.shape) for k in keys}
+        r = O.radius(g, np.arange(-G, g.n1 + G) + 0.5)
+        f["B3"][:] = (np.exp(-((r - 6.0) / 0.5) ** 2) / r)[:, None]
+        kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+        cp = lambda ks: {k: f[k].copy() for k in ks}
+        st = dict(B_prev=cp(kb), B=cp(kb), D_prev=cp(kd), D=cp(kd))
+        dt = 0.5 * (g.r_max - g.r_min) / g.n1
+        amp0 = np.abs(f["B3"]).max()
+        for _ in range(int(26.0 / dt)):
+            Bn = O.fields_prepare(g, st, dt)
+            st = O.fields_advance(g, st, Bn, None, None, dt)
+            cur = {**st["D"], **st["B"]}
+            O.field_bc(g, cur)
+            if layer:
+                O.field_match(g, cur, tgt, 10.0)
+        return np.abs(st["B"]["B3"][r < 10.0]).max() / amp0
+    assert run(False) > 0.3
+    assert run(True) < 0.02
