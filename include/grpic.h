@@ -199,9 +199,19 @@ int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic
 /* Field boundary conditions (Sec. 3.3.3), in place on D^i and B^i: the ghost columns beyond the two polar
  * axes by reflection (r- and phi-components even, theta-components odd; Fig. 1), B^2 = D^3 = 0 on the axes, and,
  * if n_const >= 0, the constant layer inside the horizon: rows i1 in [-nghost, n_const] take the values of row
- * n_const + 1 (n_const = number of current-filter passes).  The absorbing MATCH layer at the outer edge
- * (paper I) is not part of this call.  Errors: EINVAL, ECUDA. */
+ * n_const + 1 (n_const = number of current-filter passes).  The absorbing layer at the outer edge is
+ * grpic_field_match.  Errors: EINVAL, ECUDA. */
 int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const, void* cuda_stream);
+
+/* Absorbing layer at the outer radial boundary, in place on D^i and B^i: "the fields are matched to their initial
+ * values using an absorbing layer", "we smoothly match the field components with the analytic solution"
+ * (P:644).  The paper defers the profile to paper I; reading R-F6 of DESIGN.md: for r_abs < r
+ *     F <- F_target + s (F - F_target),   s = tanh(4 (r_max - r) / (r_max - r_abs)),  s = 0 for r >= r_max,
+ * with r the radius of each component's own Yee location; rows with r <= r_abs are not touched.  D_target, B_target:
+ * device arrays of the grid layout (the initial or analytic fields), read only.  r_abs in [r_min, r_max).
+ * Errors: EINVAL, ECUDA. */
+int grpic_field_match(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, const grpic_vec3* D_target, const grpic_vec3* B_target,
+                      double r_abs, void* cuda_stream);
 
 /* Current filter ("n_f passes of a digital filter"; the paper defers its form to paper I — reading R-F5 of
  * DESIGN.md): n_passes of the binomial smoothing [1 2 1]/4 along x2 and along x1, in place on J, each component on its

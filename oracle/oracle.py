@@ -4,8 +4,12 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 legs may import this module.  It never imports the CUDA package.
 
 The C file is the oracle (plain FP64 statement of PAPER.md Sec. 3.1-3.2); this module
-only marshals numpy arrays.  `sort_reference` is the one piece written in numpy: the
-sort is not in the paper, its key is defined by include/grpic.h (DESIGN.md R-S9).
+only marshals numpy arrays.  Written in numpy here: `sort_reference` (the sort is not in
+the paper, its key is defined by include/grpic.h, DESIGN.md R-S9), the time-level sequencing
+`fields_prepare` / `fields_advance` (Sec. 3.4) around the C field operators, and the boundary
+side `field_bc`, `filter_current`, `field_match` (Sec. 3.3.3).
+Parity unpinned (forms the paper defers to paper I; only their behaviour is pinned): the choice
+of digital filter in `filter_current` (R-F5) and the profile of `field_match` (R-F6).
 """
 from __future__ import annotations
 

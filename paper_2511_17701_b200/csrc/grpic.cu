@@ -684,6 +684,28 @@ int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const
   return GRPIC_OK;
 }
 
+int grpic_field_match(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, const grpic_vec3* D_target, const grpic_vec3* B_target,
+                      double r_abs, void* stream) {
+  if (!ctx) return GRPIC_EINVAL;
+  if (!D || !B || !D->F1 || !D->F2 || !D->F3 || !B->F1 || !B->F2 || !B->F3 || !D_target || !B_target ||
+      !D_target->F1 || !D_target->F2 || !D_target->F3 || !B_target->F1 || !B_target->F2 || !B_target->F3)
+    return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
+  if (!(r_abs >= ctx->r_min && r_abs < ctx->r_max)) return fail(ctx, GRPIC_EINVAL, "r_abs must be in [r_min, r_max)");
+  const FieldGeom q = make_field_geom(ctx);
+  // first array row that can lie in the layer: the cell that holds r_abs
+  double x1;
+  if (q.r_lin) x1 = (r_abs - q.r_min) / q.dr;
+  else x1 = (std::log(r_abs - q.r_off) - q.log_rmin) / q.dxi;
+  int row0 = (int)std::floor(x1) - 1 + q.ng;
+  if (row0 < 0) row0 = 0;
+  V3<real> Dv{{D->F1, D->F2, D->F3}}, Bv{{B->F1, B->F2, B->F3}};
+  CV3<real> D0{{D_target->F1, D_target->F2, D_target->F3}}, B0{{B_target->F1, B_target->F2, B_target->F3}};
+  k_field_match<real><<<dim3((q.ld + 127) / 128, q.rows - row0, 6), 128, 0, (cudaStream_t)stream>>>(
+      q, Dv, Bv, D0, B0, r_abs, ctx->r_max, row0);
+  CK(cudaGetLastError());
+  return GRPIC_OK;
+}
+
 // ---- field side of one PIC timestep (Sec. 3.4) ----
 namespace {
 int field_scratch(grpic_ctx* ctx, size_t cells) {

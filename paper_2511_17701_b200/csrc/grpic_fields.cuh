@@ -207,6 +207,28 @@ __global__ void __launch_bounds__(128) k_field_bc_layer(const FieldGeom q, const
   A[(int64_t)a1 * q.ld + a2] = A[(int64_t)(q.ng + n_const + 1) * q.ld + a2];
 }
 
+// Absorbing layer at the outer radial edge (profile in paper I -> reading R-F6): for r_abs < r the
+// field relaxes toward the target, F <- T + s (F - T), s = tanh(4 (r_max - r) / (r_max - r_abs)), s = 0 beyond r_max,
+// with r the radius of the component's own Yee location.  One thread per (row, column); blockIdx.z = component.
+template <typename T>
+__global__ void __launch_bounds__(128) k_field_match(const FieldGeom q, const V3<T> D, const V3<T> B, const CV3<T> D0,
+                                                     const CV3<T> B0, double r_abs, double r_max, int row0) {
+  const int c = blockIdx.z, a1 = row0 + blockIdx.y, a2 = threadIdx.x + blockIdx.x * blockDim.x;
+  if (a2 >= q.ld || a1 >= q.rows) return;
+  const bool half = (c == 0 || c == 4 || c == 5);            // D^1, B^2, B^3 sit at i + 1/2
+  double r, s1, th, s2;
+  field_coords(q, (double)(a1 - q.ng) + (half ? 0.5 : 0.0), 0.0, r, s1, th, s2);
+  if (!(r > r_abs)) return;
+  double d = (r_max - r) / (r_max - r_abs);
+  if (d < 0.0) d = 0.0;
+  const double s = tanh(4.0 * d);
+  T* A = c < 3 ? D.f[c] : B.f[c - 3];
+  const T* tg = c < 3 ? D0.f[c] : B0.f[c - 3];
+  const int64_t k = (int64_t)a1 * q.ld + a2;
+  const double t = (double)tg[k];
+  A[k] = (T)(t + s * ((double)A[k] - t));
+}
+
 // One pass of the binomial current filter (reading R-F5): [1 2 1]/4 along x2 then along x1 on the
 // component's own Yee lattice, mirror samples with the component's parity beyond the axes (J^1, J^3 even, J^2 odd),
 // first and last array row unchanged along x1.  in -> out (different arrays); one thread per (row, theta sample).

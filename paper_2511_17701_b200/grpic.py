@@ -23,7 +23,7 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
-           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into"]
+           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into", "grpic_field_match"]
 
 
 class GrpicError(RuntimeError):
@@ -98,6 +98,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_sorted_alive.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(C.c_int64)]
     lib.grpic_filter_current.argtypes = [_vp, C.POINTER(_Current), C.c_int32, _vp]
     lib.grpic_field_bc.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_int32, _vp]
+    lib.grpic_field_match.argtypes = [_vp] + [C.POINTER(_Vec3)] * 4 + [C.c_double, _vp]
     lib.grpic_fields_prepare.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_fields_advance.argtypes = [_vp, C.POINTER(_FieldState), C.POINTER(_Vec3), C.POINTER(_Current),
                                          C.POINTER(_Current), C.c_double, _vp]
@@ -351,6 +352,14 @@ class Context:
         d = _Vec3(*[fields[k].data_ptr() for k in ("D1", "D2", "D3")])
         b = _Vec3(*[fields[k].data_ptr() for k in ("B1", "B2", "B3")])
         self._ck(self.lib.grpic_field_bc(self.h, C.byref(d), C.byref(b), int(n_const), _stream_ptr(stream)))
+
+    def field_match(self, fields, target, r_abs, stream=None):
+        """Absorbing layer r_abs < r <= r_max: fields relax toward `target` (dict D1..B3), in place (reading R-F6)."""
+        v = lambda d, ks: _Vec3(*[d[k].data_ptr() for k in ks])
+        kb, kd = ("B1", "B2", "B3"), ("D1", "D2", "D3")
+        d, b, d0, b0 = v(fields, kd), v(fields, kb), v(target, kd), v(target, kb)
+        self._ck(self.lib.grpic_field_match(self.h, C.byref(d), C.byref(b), C.byref(d0), C.byref(b0), float(r_abs),
+                                            _stream_ptr(stream)))
 
     @staticmethod
     def _state_struct(state):

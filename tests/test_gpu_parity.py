@@ -637,6 +637,84 @@ def test_field_bc(G, O, W, prec, ng):
             assert np.array_equal(fd[k].cpu().numpy().astype(np.float64), ref[k]), (k, n_const)
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+@pytest.mark.parametrize("kw", [dict(), dict(r_map=0), dict(r0=0.4)], ids=["log", "linear", "offset"])
+def test_field_match_absorbing_layer(G, O, W, prec, kw):
+    """grpic_field_match against the oracle (reading R-F6): rows at r <= r_abs bit-unchanged, the layer rows to
+    rounding of the weight (tanh in double on both sides), rows beyond r_max = target bit for bit; three maps,
+    r_abs inside a cell, at the inner edge (whole grid is layer) and refused outside [r_min, r_max)."""
+    import torch
+    okw = dict(linear_r=1) if kw.get("r_map") == 0 else dict(kw)
+    g = O.Grid(37, 21, 0.9, 1.3, 15.0, ng=3, **okw)
+    ctx = G.Context(g.n1, g.n2, 0.9, g.r_min, g.r_max, nghost=3, precision=prec, **kw)
+    rng = np.random.default_rng(5)
+    rt = np.float32 if prec == "f32" else np.float64
+    keys = ("D1", "D2", "D3", "B1", "B2", "B3")
+    f = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in keys}
+    tg = {k: rng.normal(size=g.shape).astype(rt).astype(np.float64) for k in keys}
+    tol = 2e-7 if prec == "f32" else 1e-14
+    for r_abs in (11.3, g.r_min + 1e-9, 14.99):
+        fd = {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in f.items()}
+        td = {k: torch.from_numpy(v.astype(rt)).cuda() for k, v in tg.items()}
+        ctx.field_match(fd, td, r_abs)
+        ref = O.field_match(g, {k: v.copy() for k, v in f.items()}, tg, r_abs)
+        for k in keys:
+            got = fd[k].cpu().numpy().astype(np.float64)
+            off = 0.5 if k in ("D1", "B2", "B3") else 0.0
+            r = O.radius(g, np.arange(-g.ng, g.n1 + g.ng) + off)
+            assert np.array_equal(got[r <= r_abs], f[k][r <= r_abs]), (k, r_abs)
+            assert np.array_equal(got[r >= g.r_max * (1 + 1e-12)], tg[k][r >= g.r_max * (1 + 1e-12)]), (k, r_abs)
+            # r(x1) of the two sides agrees to a few ulp of r_max (two exponentials); the weight turns that into
+            # 4 / (r_max - r_abs) per unit of r, so a thin layer is conditioned by r_max / (r_max - r_abs)
+            bound = tol * 4.0 * max(1.0, g.r_max / (g.r_max - r_abs))
+            assert np.abs(got - ref[k]).max() <= bound, (k, r_abs, np.abs(got - ref[k]).max())
+            assert np.array_equal(td[k].cpu().numpy().astype(np.float64), tg[k])
+    for bad in (g.r_max, 0.5 * g.r_min, float("nan")):
+        with pytest.raises(G.GrpicError):
+            ctx.field_match(fd, td, bad)
+
+
+def test_vacuum_loop_with_absorbing_layer_follows_the_oracle(G, O, W):
+    """Field side of the loop with every boundary condition on the GPU (prepare, advance, axis reflection, absorbing
+    layer) against the same sequence in the oracle: flat space (App. A.1), a toroidal pulse that runs into the layer
+    and is absorbed; FP64, every 50th step compared, and the pulse is gone at the end on both sides."""
+    import torch
+    g = O.Grid(96, 8, 0.0, 2.0, 8.0, linear_r=1, mass=0.0)
+    ctx = G.Context(g.n1, g.n2, 0.0, g.r_min, g.r_max, nghost=g.ng, precision="f64", r_map=0, mass=0.0)
+    keys, kb, kd = ("D1", "D2", "D3", "B1", "B2", "B3"), ("B1", "B2", "B3"), ("D1", "D2", "D3")
+    f = {k: np.zeros(g.shape) for k in keys}
+    r = O.radius(g, np.arange(-g.ng, g.n1 + g.ng) + 0.5)
+    f["B3"][:] = (np.exp(-((r - 5.5) / 0.4) ** 2) / r)[:, None]
+    amp0 = np.abs(f["B3"]).max()
+    cp = lambda ks: {k: f[k].copy() for k in ks}
+    so = dict(B_prev=cp(kb), B=cp(kb), D_prev=cp(kd), D=cp(kd))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    sg = {n: {k: t(v) for k, v in d.items()} for n, d in so.items()}
+    zero = {k: torch.zeros(ctx.shape, dtype=torch.float64, device="cuda") for k in keys}
+    zero_o = {k: np.zeros(g.shape) for k in keys}
+    Bn = {k: torch.zeros(ctx.shape, dtype=torch.float64, device="cuda") for k in kb}
+    dt, r_abs = 0.5 * (g.r_max - g.r_min) / g.n1, 6.5
+    worst = 0.0
+    n_steps = int(14.0 / dt)
+    for step in range(1, n_steps + 1):
+        ctx.fields_prepare(sg, Bn, dt)
+        ctx.fields_advance(sg, Bn, None, None, dt)
+        cur = {**sg["D"], **sg["B"]}
+        ctx.field_bc(cur)
+        ctx.field_match(cur, zero, r_abs)
+        Bo = O.fields_prepare(g, so, dt)
+        so = O.fields_advance(g, so, Bo, None, None, dt)
+        cur_o = {**so["D"], **so["B"]}
+        O.field_bc(g, cur_o)
+        O.field_match(g, cur_o, zero_o, r_abs)
+        if step % 50 == 0 or step == n_steps:
+            for k in keys:
+                worst = max(worst, float(np.abs(cur[k].cpu().numpy() - cur_o[k]).max()) / amp0)
+    assert worst < 1e-11, worst
+    left = float(sg["B"]["B3"].abs().max()) / amp0
+    assert left < 0.03 and np.abs(so["B"]["B3"]).max() / amp0 < 0.03, left
+
+
 def test_gauss_law_is_kept_by_the_closed_loop_on_the_gpu(G, O, W):
     """"Perfect charge conservation" through the whole GPU loop in FP64: G = d_i(sqrt(h) D^i) - k_J rho~ at
     the nodes is the same after every timestep, because the deposit satisfies the discrete continuity equation
