@@ -1,6 +1,7 @@
 """A complete GRPIC run through the C ABI: config 1 ("Tiny": Kerr a = 0.9, 128x64, Wald field, e+- pairs) for a few
 hundred timesteps of the closed loop of Sec. 3.4 — fields_prepare -> fused particle step -> fields_advance -> field
-boundary conditions, with a cell sort every 10 steps.
+boundary conditions (axis reflection, constant layer inside the horizon, absorbing layer over the outer 15 % of the
+radial range matched to the initial Wald field), with a cell sort every 10 steps.
 
     python -m paper_2511_17701_b200.example [--steps 200] [--precision f32|f64] [--k_J 1e-5]
 
@@ -37,6 +38,8 @@ def main():
     B_n, J_prev = zeros(kb), zeros(kj)
     species = [G.ParticleSet.from_host(sp, prec) for sp in wl.species]
     D0 = {k: v.clone() for k, v in state["D"].items()}
+    target = {**D0, **{k: v.clone() for k, v in state["B"].items()}}   # the absorbing layer matches to the initial field
+    r_abs = dom.r_max - 0.15 * (dom.r_max - dom.r_min)
     for step in range(args.steps):
         if step % 10 == 0:
             for ps in species:
@@ -48,6 +51,7 @@ def main():
         ctx.filter_current(J, 1)
         ctx.fields_advance(state, B_n, J_prev, J, wl.dt)            # Faraday, two Ampere sub-steps
         ctx.field_bc({**state["D"], **state["B"]}, 1)               # axis reflection, constant layer inside the horizon
+        ctx.field_match({**state["D"], **state["B"]}, target, r_abs)   # absorbing layer at the outer edge
         J_prev = J
         if (step + 1) % 50 == 0 or step + 1 == args.steps:
             alive = sum(int(ps.cols["tag"].sum()) for ps in species)
