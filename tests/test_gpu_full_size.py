@@ -1,5 +1,6 @@
 """Full-size GPU checks (pytest -m gpu): BASELINE.json's configs at their real sizes, in the launch
-configuration bench.py times (grpic_sort, then the fused tiled grpic_step), checked on sampled particles
+configuration bench.py times (config 4: no *_prev columns, grpic_sort_into between two column sets, then the fused
+tiled grpic_step; configs 3 and 5: the in-place grpic_sort with all columns), checked on sampled particles
 the oracle recomputes one by one and on properties that hold at any size (discrete continuity Eq. 32/34,
 first moments, conserved u_3 and energy of geodesics)."""
 import numpy as np
@@ -59,16 +60,24 @@ def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
     rho_diff = torch.zeros(ctx.shape, dtype=torch.float64, device="cuda")
     m1 = m2 = 0.0
     scale = 0.0
+    bench_cfg = name == "large"                 # exactly what bench.py launches
     for sp in wl.species:
         ps = G.ParticleSet.from_host(sp, prec)
         n = ps.n
-        ctx.sort(ps)
+        if bench_cfg:
+            src = ps.drop_prev()
+            ps = src.empty_like()
+            ctx.sort_into(src, ps)
+            del src
+        else:
+            ctx.sort(ps)
         ctx.step(ps, fdev, J, wl.dt)            # one step to leave the freshly sorted state (drifted particles)
         for v in J.values():
             v.zero_()
         idx_np = np.unique(np.concatenate([rng.integers(0, n, 1 << 17), np.arange(0, 4096), np.arange(n - 4096, n)]))
         idx = torch.from_numpy(idx_np).cuda()
         before = _gather(ps, idx)
+        prev = {k: ps.cols[k].clone() for k in ("i1", "i2", "dx1", "dx2")}      # the position the step starts from
         ctx.step(ps, fdev, J, wl.dt)
         c = ctx.counters()
         for k in J:
@@ -79,7 +88,10 @@ def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
         op = oracle_from_cols(O, before, ps.q_over_m, ps.charge, ps.massive)
         diag = {}
         O.push(g, op, fhost, wl.dt, diag=diag)
-        res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag)
+        res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag, check_prev=not bench_cfg)
+        if not bench_cfg:                       # the *_prev columns the kernel wrote are that position
+            for k in prev:
+                assert torch.equal(ps.cols[k + "_prev"][ps.cols["tag"] != 0], prev[k][ps.cols["tag"] != 0]), k
         print(name, "full", sp.name, res, c)
         # (b) counters
         alive_after = int(ps.cols["tag"].sum())
@@ -89,16 +101,15 @@ def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
         m = ps.cols["tag"] != 0
         qw = ps.cols["weight"] * ps.charge
         rho_new = _cic_rho(torch, ctx.shape, dom.ng, ps.cols["i1"], ps.cols["i2"], ps.cols["dx1"], ps.cols["dx2"], qw, m)
-        rho_old = _cic_rho(torch, ctx.shape, dom.ng, ps.cols["i1_prev"], ps.cols["i2_prev"], ps.cols["dx1_prev"],
-                           ps.cols["dx2_prev"], qw, m)
+        rho_old = _cic_rho(torch, ctx.shape, dom.ng, prev["i1"], prev["i2"], prev["dx1"], prev["dx2"], qw, m)
         rho_diff += rho_new - rho_old
-        d1 = (ps.cols["i1"] - ps.cols["i1_prev"]).double() + (ps.cols["dx1"].double() - ps.cols["dx1_prev"].double())
-        d2 = (ps.cols["i2"] - ps.cols["i2_prev"]).double() + (ps.cols["dx2"].double() - ps.cols["dx2_prev"].double())
+        d1 = (ps.cols["i1"] - prev["i1"]).double() + (ps.cols["dx1"].double() - prev["dx1"].double())
+        d2 = (ps.cols["i2"] - prev["i2"]).double() + (ps.cols["dx2"].double() - prev["dx2"].double())
         q64 = torch.where(m, qw.double(), torch.zeros_like(d1))
         m1 += float((q64 * d1).sum()) / wl.dt
         m2 += float((q64 * d2).sum()) / wl.dt
         scale_sp = float(q64.abs().sum()) / wl.dt
-        del ps, rho_new, rho_old, d1, d2, q64
+        del ps, prev, rho_new, rho_old, d1, d2, q64
         torch.cuda.empty_cache()
     J1, J2 = Jtot["J1"], Jtot["J2"]
     div = torch.zeros_like(J1)
