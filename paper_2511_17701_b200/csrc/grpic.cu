@@ -495,7 +495,7 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
   }
   // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks (inverse permutation); 4. snapshot; 5. gather
   CK(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)sg.n_keys + 1) * 4, st));
-  k_sort_hist<<<grid_for(n), kBlock, 0, st>>>(sg, n, src->i1, src->i2, src->tag, ctx->d_keys, ctx->d_hist);
+  k_sort_hist<<<(unsigned)((n + kBlock * kSortV - 1) / (kBlock * kSortV)), kBlock, 0, st>>>(sg, n, src->i1, src->i2, src->tag, ctx->d_keys, ctx->d_hist);
   if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
 
   // tile table from the offsets (before the cursor copy is consumed)
@@ -518,7 +518,7 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
   k_items_fill<<<(n_tiles + 255) / 256, 256, 0, st>>>(ctx->d_hist, n_tiles, ctx->d_tile_items, ss.items,
                                                       ss.d_n_items, ss.d_n_items + 1);
 
-  k_sort_rank<<<grid_for(n), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
+  k_sort_rank<<<(unsigned)((n + kBlock * kSortV - 1) / (kBlock * kSortV)), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
 
   // in place: snapshot of every column in library scratch (plain contiguous copies); then ONE gather into the
   // destination columns in sorted order
@@ -551,7 +551,7 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
     CK(cudaMemcpyAsync(in.i2, p->i2, ib, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpyAsync(in.tag, p->tag, (size_t)n, cudaMemcpyDeviceToDevice, st));
   }
-  k_sort_gather<real><<<grid_for(n), kBlock, 0, st>>>(in, out, ctx->d_dest);
+  k_sort_gather<real><<<(unsigned)((n + kBlock * kGatherV - 1) / (kBlock * kGatherV)), kBlock, 0, st>>>(in, out, ctx->d_dest);
   CK(cudaGetLastError());
   // number of alive particles (they now occupy [0, n_alive)): 4 bytes read back, the one synchronisation of the sort
   uint32_t h_alive = 0;

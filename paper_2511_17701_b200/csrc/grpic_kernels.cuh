@@ -211,54 +211,110 @@ __device__ __forceinline__ uint32_t tile_key(const SortGeom& s, int i1, int i2, 
   return ((t1 * s.nt2 + t2) * kTile + l1) * kTile + l2;
 }
 
+#ifndef GRPIC_SORT_V
+#define GRPIC_SORT_V 4
+#endif
+constexpr int kSortV = GRPIC_SORT_V;       // elements per thread of the histogram and rank kernels
+
 // histogram: one atomic per run of equal keys inside a warp (sorted input -> few runs)
 __global__ void __launch_bounds__(kBlock) k_sort_hist(const SortGeom s, int64_t n, const int32_t* i1,
                                                       const int32_t* i2, const uint8_t* tag, uint32_t* key_out,
                                                       uint32_t* hist) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool in = k < n;
-  uint32_t key = 0xffffffffu;
-  if (in) {
-    key = tile_key(s, i1[k], i2[k], tag[k] != 0);
-    key_out[k] = key;
-  }
-  const unsigned peers = __match_any_sync(0xffffffffu, key);
+  // kSortV elements per thread, one block-wide stride apart: all loads are issued before the first vote
+  const int64_t k0 = (int64_t)blockIdx.x * (kBlock * kSortV) + threadIdx.x;
   const int lane = threadIdx.x & 31;
-  if (in && lane == __ffs(peers) - 1) atomicAdd(&hist[key], (uint32_t)__popc(peers));
+  uint32_t key[kSortV];
+#pragma unroll
+  for (int v = 0; v < kSortV; ++v) {
+    const int64_t k = k0 + v * kBlock;
+    key[v] = 0xffffffffu;
+    if (k < n) key[v] = tile_key(s, i1[k], i2[k], tag[k] != 0);
+  }
+#pragma unroll
+  for (int v = 0; v < kSortV; ++v) {
+    const int64_t k = k0 + v * kBlock;
+    const bool in = k < n;
+    if (in) key_out[k] = key[v];
+    const unsigned peers = __match_any_sync(0xffffffffu, key[v]);
+    if (in && lane == __ffs(peers) - 1) atomicAdd(&hist[key[v]], (uint32_t)__popc(peers));
+  }
 }
 
 // rank of every particle inside its key: offset[key]++ (warp-aggregated); written as the inverse permutation
 // src[slot] = particle, so that the move is a gather (coalesced writes, nearly sequential reads)
 __global__ void __launch_bounds__(kBlock) k_sort_rank(int64_t n, const uint32_t* key_in, uint32_t* cursor,
                                                       uint32_t* dest) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool in = k < n;
-  const uint32_t key = in ? key_in[k] : 0xffffffffu;
-  const unsigned peers = __match_any_sync(0xffffffffu, key);
+  const int64_t k0 = (int64_t)blockIdx.x * (kBlock * kSortV) + threadIdx.x;
   const int lane = threadIdx.x & 31;
-  const int leader = __ffs(peers) - 1;
-  uint32_t base = 0;
-  if (in && lane == leader) base = atomicAdd(&cursor[key], (uint32_t)__popc(peers));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  if (in) dest[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)k;   // dest[] holds the SOURCE of every slot
+  uint32_t key[kSortV], base[kSortV];
+  unsigned peers[kSortV];
+#pragma unroll
+  for (int v = 0; v < kSortV; ++v) {
+    const int64_t k = k0 + v * kBlock;
+    key[v] = k < n ? key_in[k] : 0xffffffffu;
+  }
+#pragma unroll
+  for (int v = 0; v < kSortV; ++v) {                       // the kSortV returning atomics are in flight together
+    const bool in = k0 + v * kBlock < n;
+    peers[v] = __match_any_sync(0xffffffffu, key[v]);
+    base[v] = 0;
+    if (in && lane == __ffs(peers[v]) - 1) base[v] = atomicAdd(&cursor[key[v]], (uint32_t)__popc(peers[v]));
+  }
+#pragma unroll
+  for (int v = 0; v < kSortV; ++v) {
+    const int64_t k = k0 + v * kBlock;
+    const uint32_t b = __shfl_sync(0xffffffffu, base[v], __ffs(peers[v]) - 1);
+    if (k < n) dest[b + __popc(peers[v] & ((1u << lane) - 1u))] = (uint32_t)k;   // dest[] holds the SOURCE of every slot
+  }
+}
+
+// kGatherV destination slots per thread (one block-wide stride apart, so every access of a warp stays coalesced):
+// the kGatherV source indices are loaded first and then kGatherV independent loads per column are in flight -
+// the one-slot form left the memory system latency-bound at 43 % of the DRAM rate (ncu, config 4)
+#ifndef GRPIC_GATHER_V
+#define GRPIC_GATHER_V 4
+#endif
+constexpr int kGatherV = GRPIC_GATHER_V;
+
+template <typename U>
+__device__ __forceinline__ void gather_column(U* __restrict__ dst, const U* __restrict__ from,
+                                              const uint32_t (&k)[kGatherV], const bool (&ok)[kGatherV], int64_t d0) {
+  U r[kGatherV];
+#pragma unroll
+  for (int v = 0; v < kGatherV; ++v) r[v] = from[k[v]];
+#pragma unroll
+  for (int v = 0; v < kGatherV; ++v)
+    if (ok[v]) dst[d0 + v * kBlock] = r[v];
 }
 
 template <typename T>
 __global__ void __launch_bounds__(kBlock) k_sort_gather(const PPtrs<T> in, const PPtrs<T> out,
                                                         const uint32_t* src) {
-  const int64_t d = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (d >= in.n) return;
-  const uint32_t k = src[d];
-  out.i1[d] = in.i1[k]; out.i2[d] = in.i2[k];
-  out.dx1[d] = in.dx1[k]; out.dx2[d] = in.dx2[k];
-  out.u1[d] = in.u1[k]; out.u2[d] = in.u2[k]; out.u3[d] = in.u3[k];
-  if (in.phi) out.phi[d] = in.phi[k];
-  if (in.i1p) {
-    out.i1p[d] = in.i1p[k]; out.i2p[d] = in.i2p[k];
-    out.dx1p[d] = in.dx1p[k]; out.dx2p[d] = in.dx2p[k];
+  const int64_t d0 = (int64_t)blockIdx.x * (kBlock * kGatherV) + threadIdx.x;
+  uint32_t k[kGatherV];
+  bool ok[kGatherV];
+#pragma unroll
+  for (int v = 0; v < kGatherV; ++v) {
+    const int64_t d = d0 + v * kBlock;
+    ok[v] = d < in.n;
+    k[v] = ok[v] ? src[d] : 0u;
   }
-  const_cast<T*>(out.w)[d] = in.w[k];
-  out.tag[d] = in.tag[k];
+  gather_column(out.i1, (const int32_t*)in.i1, k, ok, d0);
+  gather_column(out.i2, (const int32_t*)in.i2, k, ok, d0);
+  gather_column(out.dx1, (const T*)in.dx1, k, ok, d0);
+  gather_column(out.dx2, (const T*)in.dx2, k, ok, d0);
+  gather_column(out.u1, (const T*)in.u1, k, ok, d0);
+  gather_column(out.u2, (const T*)in.u2, k, ok, d0);
+  gather_column(out.u3, (const T*)in.u3, k, ok, d0);
+  if (in.phi) gather_column(out.phi, (const T*)in.phi, k, ok, d0);
+  if (in.i1p) {
+    gather_column(out.i1p, (const int32_t*)in.i1p, k, ok, d0);
+    gather_column(out.i2p, (const int32_t*)in.i2p, k, ok, d0);
+    gather_column(out.dx1p, (const T*)in.dx1p, k, ok, d0);
+    gather_column(out.dx2p, (const T*)in.dx2p, k, ok, d0);
+  }
+  gather_column(const_cast<T*>(out.w), in.w, k, ok, d0);
+  gather_column(out.tag, (const uint8_t*)in.tag, k, ok, d0);
 }
 
 // exclusive scan of uint32 in three passes: 1024 threads x 4 items per block
