@@ -250,6 +250,9 @@ def run_ours(args):
     J = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
     stream = torch.cuda.current_stream()
     sort_every = wl.sort_every if wl.sort_every > 0 else 10
+    # the sort orders by the cell predicted half a sort interval ahead (include/grpic.h "sort_lookahead"): the
+    # particles of a warp are then closest together in the middle of the interval, not right after the sort
+    ctx.set_real("sort_lookahead", 0.5 * sort_every)
     n_total = sum(p.n for p in sets)
 
     def one_step(it, evs=None):
@@ -349,7 +352,8 @@ def run_ours(args):
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": prec, "data": "synthetic",
         "config": {"workload": _workload_desc(wl, args.shrink), "sort_every": sort_every,
-                   "sort": "grpic_sort_into between two column sets per species; no *_prev columns (fused step)",
+                   "sort": "grpic_sort_into between two column sets per species; no *_prev columns (fused step); "
+                           "sort_lookahead = sort_every/2",
                    "l2": "inputs (particle columns, several GB) larger than the 126 MB L2; no flush needed",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "paper_context": "paper: ~1.2-1.4e8 updates/s on 1x A100 (P:550), other hardware, not a target"},

@@ -117,7 +117,15 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t value);
  * "mass":        M in units of r_g, default 1.  0 together with a = 0 gives the flat spherical metric
  *                kerr_schild_0 of App. A.1 that the paper uses for its SR-EM test.
  *                With any of these off its default every call runs the same kernels instantiated with the general coordinate
- *                class (plain evaluation of the map at every point instead of the default map's shortcuts). */
+ *                class (plain evaluation of the map at every point instead of the default map's shortcuts).
+ * "sort_lookahead": L in [0, 64] steps (default 0).  With L > 0 grpic_sort / grpic_sort_into order the particles
+ *                by the cell each is PREDICTED to occupy L steps of the last dt ahead (ballistic:
+ *                dx^i/dt = alpha h^ij u_j / gamma - beta^i of Eq. 28 at its present place, in FP32) instead of its present
+ *                cell.  An ordering heuristic only: any order is a correct sort result and grpic_step gives the same
+ *                results on it (a particle outside its tile's shared-memory window takes the global path).  With
+ *                L = half the sort interval the particles of a warp are closest together in the MIDDLE of the interval,
+ *                which the warp-level deposit aggregation rewards (config 4: -3 % per sort interval).  No effect before the
+ *                first push on the context (no dt yet). */
 int grpic_set_real(grpic_ctx* ctx, const char* key, double value);
 
 /* Steps 1-11 of Sec. 3.1 for every alive particle, then the particle boundary
@@ -144,6 +152,7 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
 
 /* Counting sort of all columns by tile-major cell key (not in the paper; north_star names it; R-S9):
  *     key = ((i1/T * ceil(n2/T) + i2/T) * T + i1%T) * T + i2%T,  T = grpic_tile_size(),
+ * of the present cell (i1, i2), or of the predicted cell when "sort_lookahead" > 0,
  * dead particles after all alive ones.  In place from the caller's view (library scratch inside).
  * Any order within one key is a correct result.  Builds the tile table that grpic_step's
  * shared-memory path uses for this species (keyed by the address of p->i1).

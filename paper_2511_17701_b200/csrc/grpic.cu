@@ -42,6 +42,7 @@ struct grpic_ctx {
   double a, r_min, r_max, small_angle, r0, h0, mass, k_J;
   int n_iter, tile_path, use_tma, early_exit;
   int64_t host_chunk;       // particles per chunk of grpic_step_host
+  double sort_lookahead;    // steps of the last dt the sort key looks ahead (0 = present cell)
   double last_dt;
   bool have_dt;
   unsigned long long* d_counters;   // 5: four of the last call + cumulative updates
@@ -241,6 +242,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->n_iter = 10;
   ctx->tile_path = 1;
   ctx->host_chunk = 1 << 22;
+  ctx->sort_lookahead = 0.0;
   ctx->use_tma = 1;
   ctx->early_exit = 1;
   ctx->have_dt = false; ctx->last_dt = 0.0;
@@ -312,6 +314,11 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
   if (!std::strcmp(key, "small_angle")) {
     if (!(v >= 0.0 && v < 1.0)) return fail(ctx, GRPIC_EINVAL, "small_angle must be in [0, 1)");
     ctx->small_angle = v;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "sort_lookahead")) {
+    if (!(v >= 0.0 && v <= 64.0)) return fail(ctx, GRPIC_EINVAL, "sort_lookahead must be in [0, 64]");
+    ctx->sort_lookahead = v;
     return GRPIC_OK;
   }
   if (!std::strcmp(key, "r0")) {
@@ -495,7 +502,17 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
   }
   // 1. keys + histogram; 2. exclusive scan -> offsets; 3. ranks (inverse permutation); 4. snapshot; 5. gather
   CK(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)sg.n_keys + 1) * 4, st));
-  k_sort_hist<<<(unsigned)((n + kBlock * kSortV - 1) / (kBlock * kSortV)), kBlock, 0, st>>>(sg, n, src->i1, src->i2, src->tag, ctx->d_keys, ctx->d_hist);
+  SortPredict sp;
+  {
+    const FieldGeom q = make_field_geom(ctx);
+    sp.on = (ctx->sort_lookahead > 0.0 && ctx->have_dt) ? 1 : 0;
+    sp.tau = sp.on ? (float)(ctx->sort_lookahead * ctx->last_dt) : 0.0f;
+    sp.log_rmin = (float)q.log_rmin; sp.dxi = (float)q.dxi; sp.r_off = (float)q.r_off; sp.r_min = (float)q.r_min;
+    sp.dr = (float)q.dr; sp.deta = (float)q.deta; sp.h0 = (float)q.h0; sp.a = (float)q.a; sp.mass = (float)q.mass;
+    sp.eps = src->massive ? 1.0f : 0.0f; sp.r_lin = q.r_lin;
+  }
+  k_sort_hist<real><<<(unsigned)((n + kBlock * kSortV - 1) / (kBlock * kSortV)), kBlock, 0, st>>>(
+      sg, sp, n, src->i1, src->i2, src->tag, src->dx1, src->dx2, src->u1, src->u2, src->u3, ctx->d_keys, ctx->d_hist);
   if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
 
   // tile table from the offsets (before the cursor copy is consumed)

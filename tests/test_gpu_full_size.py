@@ -1,6 +1,6 @@
 """Full-size GPU checks (pytest -m gpu): BASELINE.json's configs at their real sizes, in the launch
 configuration bench.py times (config 4: no *_prev columns, grpic_sort_into between two column sets, then the fused
-tiled grpic_step; configs 3 and 5: the in-place grpic_sort with all columns), checked on sampled particles
+tiled grpic_step, sort_lookahead = 5; configs 3 and 5: the in-place grpic_sort with all columns), checked on sampled particles
 the oracle recomputes one by one and on properties that hold at any size (discrete continuity Eq. 32/34,
 first moments, conserved u_3 and energy of geodesics)."""
 import numpy as np
@@ -68,6 +68,11 @@ def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
             src = ps.drop_prev()
             ps = src.empty_like()
             ctx.sort_into(src, ps)
+            ctx.set_real("sort_lookahead", 5.0)       # as bench.py: key of the cell predicted half an interval ahead
+            for _ in range(2):
+                ctx.step(ps, fdev, J, wl.dt)
+            ctx.sort_into(ps, src)
+            ps = src
             del src
         else:
             ctx.sort(ps)

@@ -332,6 +332,52 @@ def test_sort_into_and_species_without_prev_columns(G, O, W, prec):
         ctx.interp_push(cur, fdev, wl.dt)
 
 
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_sort_lookahead_gives_a_valid_order(G, O, W, prec):
+    """"sort_lookahead" orders by the cell predicted L steps ahead (a heuristic; include/grpic.h): whatever it
+    predicts, the result must be a permutation that moves every column alike, alive particles first, and the tile
+    path on that order must still agree with the oracle step by step (particles outside their tile's window take
+    the global path).  Before any step there is no dt and the order is the plain key order."""
+    wl = W.config_magnetosphere(shrink=8)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    fdev, fhost = _fields_both(G, wl, prec)
+    sp = wl.species[1]
+    rng = np.random.default_rng(13)
+    sp.tag = sp.tag.copy(); sp.tag[rng.random(sp.n) < 0.05] = 0
+    sp.weight = np.arange(1, sp.n + 1, dtype=np.float64)                     # unique id the step never changes
+    a = G.ParticleSet.from_host(sp, prec).drop_prev()
+    b = a.empty_like()
+    T = ctx.tile_size()
+    ctx.set_real("sort_lookahead", 5.0)
+    ctx.sort_into(a, b)                                                      # no dt yet: present-cell keys
+    cols = b.to_numpy()
+    key, _ = O.sort_key(g, cols["i1"], cols["i2"], cols["tag"], T)
+    assert np.all(np.diff(key) >= 0)
+    cur, other = b, a
+    for rnd in range(3):
+        for _ in range(3):
+            _one_step_parity(G, O, ctx, g, cur, fdev, fhost, wl.dt, prec, "fused")
+        before = cur.to_numpy()
+        ctx.sort_into(cur, other)
+        cur, other = other, cur
+        after = cur.to_numpy()
+        ids = after["weight"].astype(np.int64) - 1
+        ids0 = before["weight"].astype(np.int64) - 1
+        assert np.array_equal(np.sort(ids), np.arange(sp.n))
+        src_of = np.argsort(ids0)[ids]
+        for k, v in after.items():
+            if v is not None:
+                assert np.array_equal(v, before[k][src_of]), k
+        n_alive = int((before["tag"] != 0).sum())
+        assert ctx.sorted_alive(cur) == n_alive and np.all(after["tag"][:n_alive] != 0) and not after["tag"][n_alive:].any()
+        key, _ = O.sort_key(g, after["i1"], after["i2"], after["tag"], T)
+        moved = float(np.mean(np.diff(key[:n_alive].astype(np.int64)) < 0))
+        assert 0.0 < moved < 0.5                                            # predicted order: near, not equal to, the present one
+    with pytest.raises(G.GrpicError):
+        ctx.set_real("sort_lookahead", -1.0)
+
+
 def test_step_host_matches_device_step(G, O, W):
     import torch
     wl = W.config_magnetosphere(shrink=8)
