@@ -3,8 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large|...]
 
-A "step" = one pass of the whole hot path (interp + GR push + BCs + deposit, both species; grpic_sort
-every `sort_every` steps as config 4 says) over the resident particle set.  N = 1 workload:
+A "step" = one pass of the whole hot path (interp + GR push + BCs + deposit, both species; the counting sort
+every `sort_every` steps as config 4 says: grpic_sort_into between two column sets, key of the cell predicted
+sort_every/2 steps ahead) over the resident particle set.  N = 1 workload:
 BASELINE.json configs[3] "Large" (2048x1024, a = 0.9375, Wald field, ~134M e+- with density ~ r^-2,
 FP32, sort every 10 steps) — the >= 100M-particle configuration north_star's target is quoted on.
 N > 1: the path does not shard (replicas only) -> every rank runs an independent
