@@ -30,7 +30,9 @@
  *                  unity, continuity across faces);
  *   orc_deposit  — parity unpinned as to the choice among charge-conserving
  *                  schemes (pinned: discrete continuity Eq. 32/34, first
- *                  moments, one-cell hand formula).
+ *                  moments, one-cell hand formula for J^1, J^2, and the four
+ *                  node weights of J^3 of Eq. 36 written out by hand for a path
+ *                  inside one cell and for one across a face).
  */
 #define _USE_MATH_DEFINES
 #define _GNU_SOURCE

@@ -78,9 +78,15 @@ struct GlobalFieldAcc {
   }
 };
 
-// red.global.add: fire-and-forget reductions into the J arrays
-__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
-__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
+// red.global.add: fire-and-forget reductions into the J arrays.  Written as PTX on an explicit global address:
+// atomicAdd on a generic pointer makes ptxas emit, wherever it cannot prove the address space (the tiled kernels),
+// a QSPC test plus a returning ATOM and two compare-and-swap loops per call site instead of one REDG.
+__device__ __forceinline__ void red_add(float* p, float v) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "f"(v) : "memory");
+}
+__device__ __forceinline__ void red_add(double* p, double v) {
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "d"(v) : "memory");
+}
 
 // eight additions of one deposit segment (layout of deposit_segments' seg[s][0..7]) at cell offset k
 template <typename T>

@@ -137,6 +137,68 @@ def test_deposit_single_cell_hand_formula(O, g):
     assert np.count_nonzero(J["J1"]) == 2 and np.count_nonzero(J["J2"]) == 2 and np.count_nonzero(J["J3"]) == 0
 
 
+def _v3_schwarzschild(g, x1, x2, u3):
+    """Eq. 36 velocity (alpha/gamma) h^33 u_3 for a = 0, u_1 = u_2 = 0, from the textbook Schwarzschild
+    Kerr-Schild closed forms alpha = (1 + 2/r)^-1/2, h^{phi phi} = 1/(r sin theta)^2 (not from the oracle's metric)."""
+    r = g.r_min * (g.r_max / g.r_min) ** (x1 / g.n1)          # log-r map (P:820-825)
+    th = x2 * np.pi / g.n2
+    h33 = 1.0 / (r * np.sin(th)) ** 2
+    return (1.0 + 2.0 / r) ** -0.5 / np.sqrt(1.0 + h33 * u3 * u3) * h33 * u3
+
+
+def test_deposit_j3_node_weights_one_cell_hand_formula(O):
+    """Eq. 36 with J^3 located like D^3 on the nodes (i, j), reading R-S10: a particle that
+    stays in cell (5, 6) with u_3 != 0; the relay point is the midpoint of the path, each of the two half paths carries
+    q w v^3 / 2 (v^3 at the midpoint of the whole path) and puts (1-W1)(1-W2) of it on node (5, 6), W1 (1-W2) on
+    (6, 6), (1-W1) W2 on (5, 7) and W1 W2 on (6, 7), W = offsets of the half path's own midpoint.  W1 != W2
+    everywhere, so that a transposed node or swapped weights fail."""
+    gs = O.Grid(24, 16, 0.0, 2.2, 20.0)                        # a = 0
+    xa, ya, xb, yb, u3, q, w, dt = 0.2, 0.9, 0.7, 0.5, 1.7, 1.5, 2.0, 0.25
+    p = O.Particles(i1=[5], i2=[6], dx1=[xb], dx2=[yb], u1=[0.0], u2=[0.0], u3=[u3], weight=[w], tag=[1],
+                    i1_prev=[5], i2_prev=[6], dx1_prev=[xa], dx2_prev=[ya], q_over_m=1.0, charge=q)
+    J, _ = O.deposit(gs, p, dt)
+    G = gs.ng
+    xm, ym = 0.45, 0.70                                         # midpoint of the path = relay point
+    F3 = 0.5 * q * w * _v3_schwarzschild(gs, 5 + xm, 6 + ym, u3)
+    halves = ((0.5 * (xa + xm), 0.5 * (ya + ym)), (0.5 * (xm + xb), 0.5 * (ym + yb)))   # (0.325, 0.8), (0.575, 0.6)
+    want = {(5, 6): sum(F3 * (1 - W1) * (1 - W2) for W1, W2 in halves),
+            (6, 6): sum(F3 * W1 * (1 - W2) for W1, W2 in halves),
+            (5, 7): sum(F3 * (1 - W1) * W2 for W1, W2 in halves),
+            (6, 7): sum(F3 * W1 * W2 for W1, W2 in halves)}
+    assert len({round(v / F3, 12) for v in want.values()}) == 4      # four different weights
+    for (i, j), v in want.items():
+        assert np.isclose(J["J3"][i + G, j + G], v, rtol=1e-12, atol=0), (i, j)
+    assert np.count_nonzero(J["J3"]) == 4
+    assert np.isclose(J["J3"].sum(), 2 * F3, rtol=1e-13)
+
+
+def test_deposit_j3_node_weights_across_a_face_hand_formula(O):
+    """The same for a path from cell (5, 6) into cell (6, 6) (R-S10): relay point on the face x1 = 6; each of the two
+    segments carries half of q w v^3 (v^3 at the midpoint of the whole path), spread bilinearly on the four nodes
+    of ITS cell with the offsets of ITS midpoint."""
+    gs = O.Grid(24, 16, 0.0, 2.2, 20.0)
+    xa, ya, xb, yb, u3, q, w, dt = 0.8, 0.3, 0.1, 0.5, -0.9, -1.0, 3.0, 0.4     # xb is in cell 6: x = 6.1
+    p = O.Particles(i1=[6], i2=[6], dx1=[xb], dx2=[yb], u1=[0.0], u2=[0.0], u3=[u3], weight=[w], tag=[1],
+                    i1_prev=[5], i2_prev=[6], dx1_prev=[xa], dx2_prev=[ya], q_over_m=1.0, charge=q)
+    J, _ = O.deposit(gs, p, dt)
+    G = gs.ng
+    # path (5.8, 6.3) -> (6.1, 6.5); relay: x1 = 6 (the face), x2 = midpoint 6.4 (no face crossed along x2)
+    F3 = 0.5 * q * w * _v3_schwarzschild(gs, 0.5 * (5.8 + 6.1), 0.5 * (6.3 + 6.5), u3)
+    want = np.zeros(gs.shape)
+    for (c1, W1, W2) in ((5, 0.5 * (0.8 + 1.0), 0.5 * (0.3 + 0.4)),        # segment 1 in cell (5, 6)
+                         (6, 0.5 * (0.0 + 0.1), 0.5 * (0.4 + 0.5))):       # segment 2 in cell (6, 6)
+        want[c1 + G, 6 + G] += F3 * (1 - W1) * (1 - W2)
+        want[c1 + 1 + G, 6 + G] += F3 * W1 * (1 - W2)
+        want[c1 + G, 7 + G] += F3 * (1 - W1) * W2
+        want[c1 + 1 + G, 7 + G] += F3 * W1 * W2
+    assert np.allclose(J["J3"], want, rtol=1e-12, atol=1e-18)
+    assert np.count_nonzero(J["J3"]) == 6
+    # J^1 of the same path: all of it through the face-normal edge samples J1(5+1/2, .) and J1(6+1/2, .)
+    F1a, F1b = q * w * (1.0 - 0.8) / dt, q * w * 0.1 / dt
+    assert np.isclose(J["J1"][5 + G, 6 + G], F1a * (1 - 0.35)) and np.isclose(J["J1"][5 + G, 7 + G], F1a * 0.35)
+    assert np.isclose(J["J1"][6 + G, 6 + G], F1b * (1 - 0.45)) and np.isclose(J["J1"][6 + G, 7 + G], F1b * 0.45)
+
+
 def test_deposit_skips_dead_zero_charge_and_oversteps(O, g):
     rng = np.random.default_rng(7)
     p = _moved_particles(O, g, rng, 100)
