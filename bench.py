@@ -243,6 +243,9 @@ def run_ours(args):
     ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
     if args.no_tile:
         ctx.set_int("tile_path", 0)
+    for kv in args.set:                        # ablation knobs of include/grpic.h, e.g. --set lanes_path=0
+        k, v = kv.split("=", 1)
+        (ctx.set_real if k in ("sort_lookahead", "small_angle") else ctx.set_int)(k, float(v) if "." in v else int(v))
     fdev = G.grid_tensors(wl.fields, names, prec)
     # the fused step keeps the previous position in registers: no *_prev columns; two column sets per species,
     # swapped by the out-of-place sort (grpic_sort_into), so that a sort moves every byte once
@@ -396,6 +399,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--set", action="append", default=[], metavar="KEY=VALUE",
+                    help="grpic_set_int / grpic_set_real knob for ablation runs (repeatable)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -16,6 +16,7 @@
 #include "../../include/grpic.h"
 #include "grpic_kernels.cuh"
 #include "grpic_tiled.cuh"
+#include "grpic_lanes.cuh"
 #include "grpic_fields.cuh"
 
 using namespace grpic;
@@ -31,8 +32,11 @@ struct SortState {          // tile table of one species (keyed by the address o
                             // (dead at sort time, or appended later) by the direct path, so revived / injected
                             // particles are never skipped
   WorkItem* items = nullptr;
-  uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time
+  uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time, [2] dense items
+  uint32_t* dense_idx = nullptr;   // indices of the dense items (k_step_lanes), [max_items]
+  uint32_t* offsets = nullptr;     // scanned key histogram of the last sort (n_keys + 1): first slot of every sort key
   uint32_t max_items = 0;
+  uint32_t max_dense = 0;          // upper bound of [2]: grid of k_step_lanes
 };
 
 }  // namespace
@@ -41,6 +45,11 @@ struct grpic_ctx {
   grpic_grid grid;
   double a, r_min, r_max, small_angle, r0, h0, mass, k_J;
   int n_iter, tile_path, use_tma, early_exit;
+  int lanes_path;           // 1: dense work items go to k_step_lanes (grpic_lanes.cuh)
+  int64_t dense_min;        // particles from which a work item counts as dense
+  // dynamic shared-memory opt-in done on ctx->device for: k_step_lanes<real, Coord / CoordGen>,
+  // k_step_tiled<real, Coord / CoordGen, push-only / fused>, k_deposit_tiled<real, Coord / CoordGen>
+  bool lanes_attr[2], tiled_attr[2][2], dep_attr[2];
   int64_t host_chunk;       // particles per chunk of grpic_step_host
   double sort_lookahead;    // steps of the last dt the sort key looks ahead (0 = present cell)
   double last_dt;
@@ -203,6 +212,8 @@ SortGeom sort_geom(const grpic_ctx* c) {
 void free_sort_state(SortState& s) {
   if (s.items) cudaFree(s.items);
   if (s.d_n_items) cudaFree(s.d_n_items);
+  if (s.dense_idx) cudaFree(s.dense_idx);
+  if (s.offsets) cudaFree(s.offsets);
   s = SortState();
 }
 
@@ -241,6 +252,11 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->k_J = 4.0 * M_PI;                                    // coefficient of J in Ampere's law (Eq. 37)
   ctx->n_iter = 10;
   ctx->tile_path = 1;
+  ctx->lanes_path = sizeof(real) == 4 ? 1 : 0;             // FP64: measured slower than k_step_tiled (1 CTA of 256 per SM)
+  ctx->dense_min = 1024;
+  ctx->lanes_attr[0] = ctx->lanes_attr[1] = false;
+  ctx->tiled_attr[0][0] = ctx->tiled_attr[0][1] = ctx->tiled_attr[1][0] = ctx->tiled_attr[1][1] = false;
+  ctx->dep_attr[0] = ctx->dep_attr[1] = false;
   ctx->host_chunk = 1 << 22;
   ctx->sort_lookahead = 0.0;
   ctx->use_tma = 1;
@@ -291,6 +307,15 @@ int grpic_set_int(grpic_ctx* ctx, const char* key, int64_t v) {
   }
   if (!std::strcmp(key, "tile_path")) {
     ctx->tile_path = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "lanes_path")) {
+    ctx->lanes_path = v ? 1 : 0;
+    return GRPIC_OK;
+  }
+  if (!std::strcmp(key, "dense_min")) {
+    if (v < 4 || v > kChunk) return fail(ctx, GRPIC_EINVAL, "dense_min must be in 4..16384");
+    ctx->dense_min = v;
     return GRPIC_OK;
   }
   if (!std::strcmp(key, "early_exit")) {
@@ -366,9 +391,11 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
       const PPtrs<real> P = make_pptrs(p);
       const bool ok = general_map(ctx)
           ? launch_step_tiled<real, CoordGen<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
-                                                           ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
+                                                           ss.items, ss.d_n_items, ss.max_items, ss.n_alive, false,
+                                                           ctx->tiled_attr[1][0], st, terr)
           : launch_step_tiled<real, Coord<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
-                                                        ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr);
+                                                        ss.items, ss.d_n_items, ss.max_items, ss.n_alive, false,
+                                                        ctx->tiled_attr[0][0], st, terr);
       if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
       return GRPIC_OK;
     }
@@ -401,9 +428,9 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
     std::string terr;
     const bool ok = general_map(ctx)
         ? launch_deposit_tiled<real, CoordGen<real>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items,
-                                                     ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
+                                                     ss.d_n_items, ss.max_items, ss.n_alive, ctx->dep_attr[1], st, terr)
         : launch_deposit_tiled<real>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items, ss.d_n_items,
-                                     ss.max_items, ss.n_alive, st, terr);
+                                     ss.max_items, ss.n_alive, ctx->dep_attr[0], st, terr);
     if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
     return GRPIC_OK;
   }
@@ -447,10 +474,26 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   }
   const SortState& ss = it->second;
   std::string terr;
-  const bool ok = gen ? launch_step_tiled<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
-                                                                ss.items, ss.d_n_items, ss.max_items, ss.n_alive, st, terr)
-                      : launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
-                                                ss.d_n_items, ss.max_items, ss.n_alive, st, terr);
+  // dense items -> k_step_lanes (one run of particles per lane, 128-bit column blocks: every column 16-byte
+  // aligned, as include/grpic.h requires; anything else keeps all items in k_step_tiled)
+  bool lanes = ctx->lanes_path && ss.max_dense > 0;
+  {
+    const void* cols[10] = {p->i1, p->i2, p->dx1, p->dx2, p->u1, p->u2, p->u3, p->phi, p->weight, p->tag};
+    for (const void* c : cols)
+      if ((uintptr_t)c & 15u) lanes = false;
+  }
+  bool ok = gen ? launch_step_tiled<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
+                                                          ss.items, ss.d_n_items, ss.max_items, ss.n_alive, lanes,
+                                                          ctx->tiled_attr[1][1], st, terr)
+                : launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
+                                          ss.d_n_items, ss.max_items, ss.n_alive, lanes, ctx->tiled_attr[0][1], st, terr);
+  if (ok && lanes)
+    ok = gen ? launch_step_lanes<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
+                                                       ss.items, ss.dense_idx, ss.d_n_items + 2, ss.offsets,
+                                                       ss.max_dense, ctx->lanes_attr[1], st, terr)
+             : launch_step_lanes<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
+                                       ss.dense_idx, ss.d_n_items + 2, ss.offsets, ss.max_dense, ctx->lanes_attr[0],
+                                       st, terr);
   if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
   return GRPIC_OK;
 }
@@ -522,7 +565,9 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
     CK(cudaStreamSynchronize(st));
     free_sort_state(ss);
     if (cudaMalloc(&ss.items, (size_t)max_items * sizeof(WorkItem)) != cudaSuccess ||
-        cudaMalloc(&ss.d_n_items, 2 * sizeof(uint32_t)) != cudaSuccess) {
+        cudaMalloc(&ss.dense_idx, (size_t)max_items * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&ss.offsets, ((size_t)sg.n_keys + 1) * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&ss.d_n_items, 4 * sizeof(uint32_t)) != cudaSuccess) {
       cudaGetLastError();
       ctx->sorted.erase((const void*)p->i1);
       return fail(ctx, GRPIC_ENOMEM, "tile table allocation failed");
@@ -530,10 +575,15 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
     ss.max_items = max_items;
   }
   ss.n_at_sort = n;
+  // the offsets outlive this call (k_step_lanes reads them); d_hist is about to become the rank cursor
+  CK(cudaMemcpyAsync(ss.offsets, ctx->d_hist, ((size_t)sg.n_keys + 1) * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
   k_items_count<<<(n_tiles + 255) / 256, 256, 0, st>>>(ctx->d_hist, n_tiles, ctx->d_tile_items);
   if ((rc = scan_exclusive(ctx, ctx->d_tile_items, n_tiles, st))) return rc;
+  const uint32_t dense_min = ctx->lanes_path ? (uint32_t)ctx->dense_min : 0u;
+  ss.max_dense = dense_min ? (uint32_t)std::min<int64_t>(max_items, n / dense_min) : 0u;
+  CK(cudaMemsetAsync(ss.d_n_items, 0, 4 * sizeof(uint32_t), st));
   k_items_fill<<<(n_tiles + 255) / 256, 256, 0, st>>>(ctx->d_hist, n_tiles, ctx->d_tile_items, ss.items,
-                                                      ss.d_n_items, ss.d_n_items + 1);
+                                                      ss.d_n_items, ss.dense_idx, dense_min);
 
   k_sort_rank<<<(unsigned)((n + kBlock * kSortV - 1) / (kBlock * kSortV)), kBlock, 0, st>>>(n, ctx->d_keys, ctx->d_hist, ctx->d_dest);
 

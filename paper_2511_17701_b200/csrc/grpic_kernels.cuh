@@ -451,7 +451,7 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_add(uint32_t* data, uint32_
 // Work items of the tiled step: (tile, first particle, count <= kChunk).  offsets[] is the scanned
 // histogram (n_keys + 1 entries, the last two delimit the dead particles).
 struct WorkItem {
-  uint32_t tile, begin, count, pad;
+  uint32_t tile, begin, count, pad;   // pad: 1 = dense item, served by k_step_lanes
 };
 
 __global__ void k_items_count(const uint32_t* offsets, uint32_t n_tiles, uint32_t* n_items_of_tile) {
@@ -461,16 +461,24 @@ __global__ void k_items_count(const uint32_t* offsets, uint32_t n_tiles, uint32_
   n_items_of_tile[t] = (cnt + kChunk - 1) / kChunk;
 }
 
+// dense_min > 0: items of at least dense_min particles are marked (pad = 1) and listed in dense_idx for
+// k_step_lanes (grpic_lanes.cuh); k_step_tiled then leaves them alone.  n_out: [0] items, [1] alive, [2] dense items
+// ([2] zeroed by the caller).
 __global__ void k_items_fill(const uint32_t* offsets, uint32_t n_tiles, const uint32_t* item_offset_of_tile,
-                             WorkItem* items, uint32_t* n_items_out, uint32_t* n_alive_out) {
+                             WorkItem* items, uint32_t* n_out, uint32_t* dense_idx, uint32_t dense_min) {
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_tiles) return;
   const uint32_t b = offsets[t * kTile * kTile], e = offsets[(t + 1) * kTile * kTile];
   uint32_t k = item_offset_of_tile[t];
-  for (uint32_t s = b; s < e; s += kChunk) items[k++] = WorkItem{t, s, min((uint32_t)kChunk, e - s), 0u};
+  for (uint32_t s = b; s < e; s += kChunk) {
+    const uint32_t cnt = min((uint32_t)kChunk, e - s);
+    const uint32_t dense = (dense_min > 0u && cnt >= dense_min) ? 1u : 0u;
+    if (dense) dense_idx[atomicAdd(&n_out[2], 1u)] = k;
+    items[k++] = WorkItem{t, s, cnt, dense};
+  }
   if (t == n_tiles - 1) {
-    *n_items_out = k;
-    *n_alive_out = e;
+    n_out[0] = k;
+    n_out[1] = e;
   }
 }
 

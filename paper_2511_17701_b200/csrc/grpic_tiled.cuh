@@ -307,7 +307,7 @@ template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
-                 uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma,
+                 uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma, int skip_dense,
                  const __grid_constant__ FieldMaps maps) {
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the kWarps private J tiles
@@ -326,6 +326,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   }
   if (blockIdx.x >= n_items_ptr[0]) return;
   const WorkItem item = items[blockIdx.x];
+  if (skip_dense && item.pad) return;                 // a dense item: k_step_lanes has it (grpic_lanes.cuh)
   const int c1lo = (int)(item.tile / (uint32_t)nt2) * kTile - kHalo;   // window origin, cells
   const int c2lo = (int)(item.tile % (uint32_t)nt2) * kTile - kHalo;
   // first fetched column (array index): the window's first sample, rounded down to a multiple of 4
@@ -624,8 +625,8 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
 template <typename T, typename CoordT = Coord<T>>
 bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>& J, const SpeciesConst& sc,
                           unsigned long long* counters, const WorkItem* items, const uint32_t* d_n_items,
-                          uint32_t max_items, int64_t n_covered, cudaStream_t st, std::string& err) {
-  static bool attr_set = false;
+                          uint32_t max_items, int64_t n_covered, bool& attr_set, cudaStream_t st, std::string& err) {
+  // attr_set: the shared-memory opt-in is per device and per loaded module; the flag lives in the context
   if (!attr_set) {
     cudaError_t ea = cudaFuncSetAttribute(k_deposit_tiled<T, CoordT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)deposit_smem_bytes<T>());
@@ -652,8 +653,7 @@ template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
                        const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
-                       cudaStream_t st, std::string& err) {
-  static bool attr_set = false;
+                       bool skip_dense, bool& attr_set, cudaStream_t st, std::string& err) {
   if (!attr_set) {
     cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T, CoordT, kDeposit>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)tiled_smem_bytes<T>());
@@ -673,7 +673,7 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
   const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
   k_step_tiled<T, CoordT, kDeposit><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
-                                                                n_at_sort, nt2, use_tma, maps);
+                                                                n_at_sort, nt2, use_tma, skip_dense ? 1 : 0, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     err = std::string("k_step_tiled launch: ") + cudaGetErrorString(e);
