@@ -42,7 +42,8 @@ static_assert(kLVals * kLThreads >= kRawElems, "the raw field stencil is staged 
 
 template <typename T>
 constexpr size_t lanes_smem_bytes() {
-  return (size_t)(kLVals * kLThreads + kNodeElems + 7 * 4 * kLThreads) * sizeof(T) + (size_t)(2 * 4 + 1) * kLThreads * 4 + 16;
+  return (size_t)(kLVals * kLThreads + kNodeElems + 7 * 4 * kLThreads) * sizeof(T) + (size_t)(2 * 4 + 1) * kLThreads * 4 + 16 +
+         (size_t)(kTile * kTile + 4) * 4;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -71,6 +72,25 @@ __device__ __forceinline__ void lane_add8(T* pW, int c1, int c2, const T v[8]) {
   p00[32 * S] += v[4];   p10[32 * S] += v[5];            // J3(c1, c2), J3(c1+1, c2)
   p01[32 * S] += v[6];   p11[32 * S] += v[7];            // J3(c1, c2+1), J3(c1+1, c2+1)
 }
+
+// The same in two halves, so that the eight loads can be issued ahead of the arithmetic that produces the addends
+template <typename T>
+struct LaneCell {
+  T *p00, *p01, *p10, *p11;
+  T o[8];
+  __device__ __forceinline__ void load(T* pW, int c1, int c2) {
+    constexpr int S = kLThreads;
+    const int r0 = (c1 & 3) * 4, r1 = ((c1 + 1) & 3) * 4, q0 = c2 & 3, q1 = (c2 + 1) & 3;
+    p00 = pW + (r0 + q0) * S; p01 = pW + (r0 + q1) * S; p10 = pW + (r1 + q0) * S; p11 = pW + (r1 + q1) * S;
+    o[0] = p00[0]; o[1] = p01[0]; o[2] = p00[16 * S]; o[3] = p10[16 * S];
+    o[4] = p00[32 * S]; o[5] = p10[32 * S]; o[6] = p01[32 * S]; o[7] = p11[32 * S];
+  }
+  __device__ __forceinline__ void add_store(const T v[8]) const {
+    constexpr int S = kLThreads;
+    p00[0] = o[0] + v[0]; p01[0] = o[1] + v[1]; p00[16 * S] = o[2] + v[2]; p10[16 * S] = o[3] + v[3];
+    p00[32 * S] = o[4] + v[4]; p10[32 * S] = o[5] + v[5]; p01[32 * S] = o[6] + v[6]; p11[32 * S] = o[7] + v[7];
+  }
+};
 
 // node (n1, n2) of the lane's window: its three non-zero slots go to the J arrays with red.global.add and are zeroed.
 // No bounds test: a slot whose node lies outside the arrays is never written (no cell there), so it stays zero.
@@ -113,6 +133,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   int32_t* sI = reinterpret_cast<int32_t*>(sR + 7 * 4 * NT);   // staged cell indices [2][thread][4]
   uint32_t* sT = reinterpret_cast<uint32_t*>(sI + 2 * 4 * NT); // staged tags: four bytes per thread
   uint64_t* bar = reinterpret_cast<uint64_t*>(sT + NT);
+  uint32_t* sO = reinterpret_cast<uint32_t*>(bar + 2);         // first slot of each of the tile's 256 sort keys, + end
 
   if (blockIdx.x >= n_dense_ptr[0]) return;
   const int tid = threadIdx.x;
@@ -122,6 +143,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   const int a2lo = c2lo - 1 + g.ng;
   const int off2 = ((a2lo % 4) + 4) % 4;
 
+  for (int e = tid; e <= kTile * kTile; e += NT) sO[e] = __ldg(offsets + (size_t)item.tile * (kTile * kTile) + e);
   // ---- 1. stage the field stencil (as k_step_tiled) ----
   if (use_tma) {
     if (tid == 0) {
@@ -182,7 +204,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   // pass in the middle of the sort interval, around which they are spread evenly before and after.
   bool have_win = false;
   int wo1 = 0, wo2 = 0;                                // window origin (cell): cells wo .. wo + 2, nodes wo .. wo + 3
-  const uint32_t* const offs = offsets + (size_t)item.tile * (kTile * kTile);   // keys of this tile: offs[0 .. 256]
+  const uint32_t* const offs = sO;                     // keys of this tile: offs[0 .. 256]
   uint32_t key = 0, next_b = 0;
   if (b_first < B1) {                                  // key of the run's first particle: offs[key] <= k < offs[key + 1]
     const uint32_t kf = max(b_first << 2, begin);
@@ -190,10 +212,10 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
 #pragma unroll 1
     while (hi - lo > 1u) {
       const uint32_t mid = (lo + hi) >> 1;
-      if (__ldg(offs + mid) <= kf) lo = mid; else hi = mid;
+      if (offs[mid] <= kf) lo = mid; else hi = mid;
     }
     key = lo;
-    next_b = __ldg(offs + key + 1);
+    next_b = offs[key + 1];
   }
   const int t1c = (int)(item.tile / (uint32_t)nt2) * kTile, t2c = (int)(item.tile % (uint32_t)nt2) * kTile;
   const T* const rcol[7] = {P.dx1, P.dx2, P.u1, P.u2, P.u3, P.phi, P.w};
@@ -204,7 +226,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
     const bool full = k0 >= begin && k0 + 4u <= end;
     {                                                  // move the window to the sorted cell of this block
       const uint32_t kb = max(k0, begin);
-      while (kb >= next_b) { ++key; next_b = __ldg(offs + key + 1); }
+      while (kb >= next_b) { ++key; next_b = offs[key + 1]; }
       const int n1 = t1c + (int)(key >> 4) - 1, n2 = t2c + (int)(key & 15u) - 1;
       if (have_win && (n1 != wo1 || n2 != wo2)) {
         if (n1 == wo1 && n2 == wo2 + 1) lane_flush_col(g, J, pW, wo1, wo2);
@@ -265,25 +287,31 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
       if (P.i1p) { P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya; }
       const int wa1 = ia - c1lo, wa2 = ja - c2lo;      // cell inside the field window?
       const bool a_in = (unsigned)wa1 < (unsigned)kWinC && (unsigned)wa2 < (unsigned)kWinC;
-      const int64_t cell = (int64_t)(ia + g.ng) * g.ld + (ja + g.ng);
       T Dp[3], Bp[3];
       if (a_in) {
         interp_nodes(sN, wa1 * kNodeW + wa2, p.dx1, p.dx2, Dp, Bp);
       } else {
-        GlobalFieldAcc<T> acc{F, cell, g.ld};
+        GlobalFieldAcc<T> acc{F, (int64_t)(ia + g.ng) * g.ld + (ja + g.ng), g.ld};
         interp_fields(acc, p.dx1, p.dx2, Dp, Bp);
       }
       T dphidt;
       bool reflected;
       const int res = push_particle<T, CoordT>(g, p, true, Dp, Bp, (T)sc.q_over_m, eps, dt, dphidt, reflected);
+      n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
+      const int di = p.i1 - ia, dj = p.i2 - ja;
+      const bool over = di > 1 || di < -1 || dj > 1 || dj < -1;
+      const bool dep = res == 0 && !over;
+      // the window slots of the start cell are requested now; the write-back of the particle and the arithmetic of
+      // the deposit run while they arrive
+      const bool a_win = dep && (unsigned)(ia - wo1) < (unsigned)kLWin && (unsigned)(ja - wo2) < (unsigned)kLWin;
+      LaneCell<T> wa;
+      if (a_win) wa.load(pW, ia, ja);
       myI[s] = p.i1; myI[4 * NT + s] = p.i2;
       myR[s] = p.dx1; myR[4 * NT + s] = p.dx2;
       myR[2 * 4 * NT + s] = p.u1; myR[3 * 4 * NT + s] = p.u2; myR[4 * 4 * NT + s] = p.u3;
       if (sc.has_phi) myR[5 * 4 * NT + s] += dt * dphidt;
-      n_alive += (res == 0); n_in += (res == 1); n_out += (res == 2);
       if (res != 0) { tags &= ~(0xffu << (8 * s)); continue; }
-      const int di = p.i1 - ia, dj = p.i2 - ja;
-      if (di > 1 || di < -1 || dj > 1 || dj < -1) { ++n_over; continue; }
+      if (over) { ++n_over; continue; }
       T v3 = dphidt;
       if (reflected)
         v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2),
@@ -297,16 +325,16 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
         for (int q = 0; q < 8; ++q) seg[0][q] += seg[1][q];
       }
       // into the lane's window where the path lies inside it; a stray (drift since the sort) goes to L2 directly
-      if ((unsigned)(ia - wo1) < (unsigned)kLWin && (unsigned)(ja - wo2) < (unsigned)kLWin)
-        lane_add8(pW, ia, ja, seg[0]);
+      if (a_win)
+        wa.add_store(seg[0]);
       else
-        global_add8(J, cell, g.ld, seg[0]);
+        global_add8(J, (int64_t)(ia + g.ng) * g.ld + (ja + g.ng), g.ld, seg[0]);
       if (cross) {
         const int ib = ia + di, jb = ja + dj;
         if ((unsigned)(ib - wo1) < (unsigned)kLWin && (unsigned)(jb - wo2) < (unsigned)kLWin)
           lane_add8(pW, ib, jb, seg[1]);
         else
-          global_add8(J, cell + (int64_t)di * g.ld + dj, g.ld, seg[1]);
+          global_add8(J, (int64_t)(ib + g.ng) * g.ld + (jb + g.ng), g.ld, seg[1]);
       }
     }
     // ---- stage out ----
