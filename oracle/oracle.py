@@ -352,6 +352,10 @@ def fields_prepare(g: Grid, state: dict, dt: float) -> dict:
     E_half = aux_fields(g, {**state["B"], **D_half})                    # (n-1/2)E from (n-1/2)B, (n-1/2)D
     B_n = {k: np.array(v) for k, v in B_nm1.items()}
     faraday(g, B_n, E_half, dt)                                         # (n-1)B -> (n)B
+    # Boundary conditions are imposed on the evolved field components, and the ghost zones next to the axis satisfy
+    # reflection symmetry: the push reads the ghost columns of (n)B, which Faraday does not write
+    if g.n2 >= g.ng:
+        _axis_reflect(g, B_n)
     return B_n
 
 
@@ -382,8 +386,19 @@ _AXIS_PARITY = {"D1": (+1, 0.0), "D2": (-1, 0.5), "D3": (+1, 0.0), "B1": (+1, 0.
 def field_bc(g: Grid, fields: dict, n_const: int = -1) -> dict:
     """In place on dict(D1..B3) of float64 arrays; n_const >= 0: rows i1 in [-ng, n_const] take the values of row
     n_const + 1 (n_const = number of current-filter passes n_f)."""
+    _axis_reflect(g, fields)
+    if n_const >= 0:
+        for A in fields.values():
+            A[: g.ng + n_const + 1, :] = A[g.ng + n_const + 1, :]
+    return fields
+
+
+def _axis_reflect(g: Grid, fields: dict) -> None:
+    """ghost columns beyond the two polar axes of whichever of D1..B3 are in `fields`, and the zeros on the axes"""
     G, n2 = g.ng, g.n2
     for k, (par, off) in _AXIS_PARITY.items():
+        if k not in fields:
+            continue
         A = fields[k]
         for m in range(1, G + 1):
             if off == 0.0:                       # samples at integer j: ghost j = -m mirrors j = +m; j = n2+m mirrors n2-m
@@ -394,12 +409,9 @@ def field_bc(g: Grid, fields: dict, n_const: int = -1) -> dict:
                 A[:, G - m] = par * A[:, G + m - 1]
                 A[:, G + n2 + m - 1] = par * A[:, G + n2 - m]
     for k in ("B2", "D3"):                       # vanish on the axes by symmetry
-        fields[k][:, G] = 0.0
-        fields[k][:, G + n2] = 0.0
-    if n_const >= 0:
-        for A in fields.values():
-            A[: G + n_const + 1, :] = A[G + n_const + 1, :]
-    return fields
+        if k in fields:
+            fields[k][:, G] = 0.0
+            fields[k][:, G + n2] = 0.0
 
 
 # ----------------------------------------------------------------------------------------------

@@ -28,9 +28,12 @@ std::string g_create_error;
 
 struct SortState {          // tile table of one species (keyed by the address of its i1 column)
   int64_t n_at_sort = 0;    // p->n when the table was built
-  int64_t n_alive = 0;      // alive particles at that time: slots [0, n_alive) are covered by the table, the rest
-                            // (dead at sort time, or appended later) by the direct path, so revived / injected
-                            // particles are never skipped
+  // Alive particles at that time, d_n_items[1] on the device: slots [0, n_alive) are covered by the table, the rest
+  // (dead at sort time, or appended later) by the direct path, so revived / injected particles are never skipped.
+  // The host copy is fetched only when somebody asks (grpic_sorted_alive, or a call with p->n < n_at_sort).
+  int64_t n_alive = 0;
+  bool n_alive_known = false;
+  cudaStream_t stream = nullptr;   // stream of the sort (the read-back waits on it)
   WorkItem* items = nullptr;
   uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time, [2] dense items
   uint32_t* dense_idx = nullptr;   // indices of the dense items (k_step_lanes), [max_items]
@@ -90,6 +93,15 @@ int cuda_fail(grpic_ctx* c, cudaError_t e, const char* what) {
     cudaError_t e_ = (call);                                  \
     if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);  \
   } while (0)
+
+// Every buffer, the tile tables and the shared-memory opt-ins of a context belong to the device that was current at
+// grpic_create: a call made with another device current is refused rather than launched on the wrong GPU.
+int check_device(grpic_ctx* ctx) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device)
+    return fail(ctx, GRPIC_ESTATE, "the current CUDA device is not the one this context was created on");
+  return GRPIC_OK;
+}
 
 Consts<real> make_consts(const grpic_ctx* c) {
   Consts<real> g;
@@ -208,6 +220,28 @@ SortGeom sort_geom(const grpic_ctx* c) {
   s.n_keys = (uint32_t)s.nt1 * s.nt2 * kTile * kTile + 1u;
   return s;
 }
+
+// host copy of the alive count of the last sort (synchronises the stream of that sort, once)
+int fetch_alive(grpic_ctx* ctx, SortState& s) {
+  if (s.n_alive_known) return GRPIC_OK;
+  uint32_t h = 0;
+  CK(cudaMemcpyAsync(&h, s.d_n_items + 1, sizeof(uint32_t), cudaMemcpyDeviceToHost, s.stream));
+  CK(cudaStreamSynchronize(s.stream));
+  s.n_alive = (int64_t)h;
+  s.n_alive_known = true;
+  return GRPIC_OK;
+}
+
+// May the tile table of `s` serve a call on p?  Yes while p still has every slot the table covers: always if p->n has
+// not shrunk since the sort; after a compaction (p->n lowered towards the alive count) the count is fetched once.
+bool table_covers(grpic_ctx* ctx, SortState& s, const grpic_particles* p) {
+  if (p->n >= s.n_at_sort) return true;
+  if (fetch_alive(ctx, s) != GRPIC_OK) return false;
+  return s.n_alive <= p->n;
+}
+
+// grid of the kernels that walk the slots behind the alive count (k_*_from): fixed, block-strided
+constexpr unsigned kTailGrid = 148 * 4;
 
 void free_sort_state(SortState& s) {
   if (s.items) cudaFree(s.items);
@@ -370,6 +404,7 @@ int grpic_set_real(grpic_ctx* ctx, const char* key, double v) {
 
 int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, p, 1);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
@@ -383,7 +418,7 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
   JPtrs<real> J{{nullptr, nullptr, nullptr}};
   {
     auto it = ctx->sorted.find((const void*)p->i1);
-    if (ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n && sc.em) {
+    if (ctx->tile_path && it != ctx->sorted.end() && sc.em && table_covers(ctx, it->second, p)) {
       // sorted species: field stencil of each tile staged in shared memory, as in the fused step
       const SortState& ss = it->second;
       std::string terr;
@@ -391,12 +426,18 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
       const PPtrs<real> P = make_pptrs(p);
       const bool ok = general_map(ctx)
           ? launch_step_tiled<real, CoordGen<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
-                                                           ss.items, ss.d_n_items, ss.max_items, ss.n_alive, false,
+                                                           ss.items, ss.d_n_items, ss.max_items, false,
                                                            ctx->tiled_attr[1][0], st, terr)
           : launch_step_tiled<real, Coord<real>, false>(ctx->tma, ctx->use_tma != 0, g, P, F, J, sc, ctx->d_counters,
-                                                        ss.items, ss.d_n_items, ss.max_items, ss.n_alive, false,
+                                                        ss.items, ss.d_n_items, ss.max_items, false,
                                                         ctx->tiled_attr[0][0], st, terr);
       if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
+      if (general_map(ctx))
+        k_push_or_step_from<real, false, CoordGen<real>><<<kTailGrid, kBlock, 0, st>>>(g, P, F, J, sc, ctx->d_counters,
+                                                                                       ss.d_n_items + 1);
+      else
+        k_push_or_step_from<real, false><<<kTailGrid, kBlock, 0, st>>>(g, P, F, J, sc, ctx->d_counters, ss.d_n_items + 1);
+      CK(cudaGetLastError());
       return GRPIC_OK;
     }
   }
@@ -412,6 +453,7 @@ int grpic_interp_push(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fi
 
 int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, p, 1);
   if (rc) return rc;
   if (!ctx->have_dt) return fail(ctx, GRPIC_ESTATE, "grpic_deposit before any grpic_interp_push on this context");
@@ -422,16 +464,23 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
   CK(cudaMemsetAsync(ctx->d_counters + 3, 0, sizeof(unsigned long long), st));
   if (p->n == 0 || !sc.do_deposit) return GRPIC_OK;
   auto it = ctx->sorted.find((const void*)p->i1);
-  if (ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n) {
+  if (ctx->tile_path && it != ctx->sorted.end() && table_covers(ctx, it->second, p)) {
     // sorted species: per-warp shared J tiles and warp aggregation instead of one L2 reduction per contribution
     const SortState& ss = it->second;
     std::string terr;
     const bool ok = general_map(ctx)
         ? launch_deposit_tiled<real, CoordGen<real>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items,
-                                                     ss.d_n_items, ss.max_items, ss.n_alive, ctx->dep_attr[1], st, terr)
+                                                     ss.d_n_items, ss.max_items, ctx->dep_attr[1], st, terr)
         : launch_deposit_tiled<real>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters, ss.items, ss.d_n_items,
-                                     ss.max_items, ss.n_alive, ctx->dep_attr[0], st, terr);
+                                     ss.max_items, ctx->dep_attr[0], st, terr);
     if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
+    if (general_map(ctx))
+      k_deposit_from<real, CoordGen<real>><<<kTailGrid, kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc,
+                                                                         ctx->d_counters, ss.d_n_items + 1);
+    else
+      k_deposit_from<real><<<kTailGrid, kBlock, 0, st>>>(make_consts(ctx), make_pptrs(p), Jp, sc, ctx->d_counters,
+                                                         ss.d_n_items + 1);
+    CK(cudaGetLastError());
     return GRPIC_OK;
   }
   if (general_map(ctx))
@@ -445,6 +494,7 @@ int grpic_deposit(grpic_ctx* ctx, const grpic_particles* p, grpic_current* J, vo
 int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, grpic_current* J, double dt,
                void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, p, 2);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(ctx, GRPIC_EINVAL, "dt must be > 0");
@@ -461,8 +511,8 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
   const PPtrs<real> P = make_pptrs(p);
 
   auto it = ctx->sorted.find((const void*)p->i1);
-  const bool tiled = ctx->tile_path && it != ctx->sorted.end() && it->second.n_alive <= p->n && sc.em &&
-                     sc.do_deposit;
+  const bool tiled = ctx->tile_path && it != ctx->sorted.end() && sc.em && sc.do_deposit &&
+                     table_covers(ctx, it->second, p);
   const bool gen = general_map(ctx);             // full A.3 map (r0, h0): same kernels, general coordinate class
   if (!tiled) {
     if (gen)
@@ -483,10 +533,10 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
       if ((uintptr_t)c & 15u) lanes = false;
   }
   bool ok = gen ? launch_step_tiled<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
-                                                          ss.items, ss.d_n_items, ss.max_items, ss.n_alive, lanes,
+                                                          ss.items, ss.d_n_items, ss.max_items, lanes,
                                                           ctx->tiled_attr[1][1], st, terr)
                 : launch_step_tiled<real>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters, ss.items,
-                                          ss.d_n_items, ss.max_items, ss.n_alive, lanes, ctx->tiled_attr[0][1], st, terr);
+                                          ss.d_n_items, ss.max_items, lanes, ctx->tiled_attr[0][1], st, terr);
   if (ok && lanes)
     ok = gen ? launch_step_lanes<real, CoordGen<real>>(ctx->tma, ctx->use_tma != 0, g, P, F, Jp, sc, ctx->d_counters,
                                                        ss.items, ss.dense_idx, ss.d_n_items + 2, ss.offsets,
@@ -495,6 +545,13 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
                                        ss.dense_idx, ss.d_n_items + 2, ss.offsets, ss.max_dense, ctx->lanes_attr[0],
                                        st, terr);
   if (!ok) return fail(ctx, GRPIC_ECUDA, terr);
+  // slots behind the alive count of the sort (dead then; revived or appended since): direct path
+  if (gen)
+    k_push_or_step_from<real, true, CoordGen<real>><<<kTailGrid, kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters,
+                                                                                  ss.d_n_items + 1);
+  else
+    k_push_or_step_from<real, true><<<kTailGrid, kBlock, 0, st>>>(g, P, F, Jp, sc, ctx->d_counters, ss.d_n_items + 1);
+  CK(cudaGetLastError());
   return GRPIC_OK;
 }
 
@@ -620,17 +677,16 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
   }
   k_sort_gather<real><<<(unsigned)((n + kBlock * kGatherV - 1) / (kBlock * kGatherV)), kBlock, 0, st>>>(in, out, ctx->d_dest);
   CK(cudaGetLastError());
-  // number of alive particles (they now occupy [0, n_alive)): 4 bytes read back, the one synchronisation of the sort
-  uint32_t h_alive = 0;
-  CK(cudaMemcpyAsync(&h_alive, ss.d_n_items + 1, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  ss.n_alive = (int64_t)h_alive;
+  // the number of alive particles (they now occupy [0, n_alive)) stays on the device: the kernels read it there
+  ss.n_alive_known = false;
+  ss.stream = st;
   return GRPIC_OK;
 }
 }  // namespace
 
 int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, p, 2);
   if (rc) return rc;
   return sort_impl(ctx, p, p, (cudaStream_t)stream);
@@ -638,6 +694,7 @@ int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* stream) {
 
 int grpic_sort_into(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* dst, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, src, 2);
   if (rc || (rc = check_particles(ctx, dst, 2))) return rc;
   if (src->n != dst->n) return fail(ctx, GRPIC_EINVAL, "sort_into: src.n != dst.n");
@@ -659,6 +716,8 @@ int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_aliv
   if (!ctx || !p || !n_alive) return fail(ctx, GRPIC_EINVAL, "NULL argument");
   auto it = ctx->sorted.find((const void*)p->i1);
   if (it == ctx->sorted.end()) return fail(ctx, GRPIC_ESTATE, "this species has not been sorted on this context");
+  int rc = fetch_alive(ctx, it->second);
+  if (rc) return rc;
   *n_alive = it->second.n_alive;
   return GRPIC_OK;
 }
@@ -689,6 +748,7 @@ int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* stream) {
 // ------------------------------------------------------------------------------------------------
 int grpic_aux_fields(grpic_ctx* ctx, const grpic_fields* em, grpic_vec3* E, grpic_vec3* H, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!em || !em->D1 || !em->D2 || !em->D3 || !em->B1 || !em->B2 || !em->B3)
     return fail(ctx, GRPIC_EINVAL, "a field component pointer is NULL");
   if (!E && !H) return fail(ctx, GRPIC_EINVAL, "both outputs are NULL");
@@ -707,6 +767,7 @@ int grpic_aux_fields(grpic_ctx* ctx, const grpic_fields* em, grpic_vec3* E, grpi
 
 int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!B || !E || !B->F1 || !B->F2 || !B->F3 || !E->F1 || !E->F2 || !E->F3)
     return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
   const FieldGeom q = make_field_geom(ctx);
@@ -721,6 +782,7 @@ int grpic_faraday(grpic_ctx* ctx, grpic_vec3* B, const grpic_vec3* E, double dt,
 
 int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic_current* J, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!D || !H || !D->F1 || !D->F2 || !D->F3 || !H->F1 || !H->F2 || !H->F3)
     return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
   if (J && (!J->J1 || !J->J2 || !J->J3)) return fail(ctx, GRPIC_EINVAL, "a current component pointer is NULL");
@@ -737,6 +799,7 @@ int grpic_ampere(grpic_ctx* ctx, grpic_vec3* D, const grpic_vec3* H, const grpic
 
 int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!D || !B || !D->F1 || !D->F2 || !D->F3 || !B->F1 || !B->F2 || !B->F3)
     return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
   const FieldGeom q = make_field_geom(ctx);
@@ -744,7 +807,7 @@ int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const
   if (q.n2 < q.ng) return fail(ctx, GRPIC_EINVAL, "n2 must be >= nghost for the axis reflection");
   V3<real> Dv{{D->F1, D->F2, D->F3}}, Bv{{B->F1, B->F2, B->F3}};
   cudaStream_t st = (cudaStream_t)stream;
-  k_field_bc_axis<real><<<dim3(1, q.rows, 6), 128, 0, st>>>(q, Dv, Bv);
+  k_field_bc_axis<real><<<dim3(1, q.rows, 6), 128, 0, st>>>(q, Dv, Bv, 0);
   if (n_const >= 0)
     k_field_bc_layer<real><<<dim3((q.ld + 127) / 128, q.ng + n_const + 1, 6), 128, 0, st>>>(q, Dv, Bv, n_const);
   CK(cudaGetLastError());
@@ -754,6 +817,7 @@ int grpic_field_bc(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, int32_t n_const
 int grpic_field_match(grpic_ctx* ctx, grpic_vec3* D, grpic_vec3* B, const grpic_vec3* D_target, const grpic_vec3* B_target,
                       double r_abs, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!D || !B || !D->F1 || !D->F2 || !D->F3 || !B->F1 || !B->F2 || !B->F3 || !D_target || !B_target ||
       !D_target->F1 || !D_target->F2 || !D_target->F3 || !B_target->F1 || !B_target->F2 || !B_target->F3)
     return fail(ctx, GRPIC_EINVAL, "a component pointer is NULL");
@@ -797,6 +861,7 @@ void average3(real* out, const real* a1, const real* a2, const real* a3, const r
 
 int grpic_filter_current(grpic_ctx* ctx, grpic_current* J, int32_t n_passes, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!J || !J->J1 || !J->J2 || !J->J3) return fail(ctx, GRPIC_EINVAL, "a current component pointer is NULL");
   if (n_passes < 0) return fail(ctx, GRPIC_EINVAL, "n_passes must be >= 0");
   const FieldGeom q = make_field_geom(ctx);
@@ -820,6 +885,7 @@ int grpic_filter_current(grpic_ctx* ctx, grpic_current* J, int32_t n_passes, voi
 
 int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3* B_n, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!s || !vec3_ok(&s->B_prev) || !vec3_ok(&s->B) || !vec3_ok(&s->D_prev) || !vec3_ok(&s->D) || !vec3_ok(B_n))
     return fail(ctx, GRPIC_EINVAL, "a field pointer is NULL");
   const FieldGeom q = make_field_geom(ctx);
@@ -845,6 +911,13 @@ int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3*
     CV3<real> Ec{{E, E + cells, E + 2 * cells}};
     k_faraday<real><<<dim3((q.n2 + 127) / 128, q.rows - 4), 128, 0, st>>>(q, Bv, Ec, dt);
   }
+  // (n)B is what the particle gather reads, ghost columns beyond the axes included (node averages of B^1, B^3 in
+  // the cells next to an axis): Faraday wrote the physical columns only, so the axis reflection is applied
+  // to (n)B here - otherwise its ghost columns would still hold the time level n-1
+  if (q.n2 >= q.ng) {
+    V3<real> Bv{{B_n->F1, B_n->F2, B_n->F3}};
+    k_field_bc_axis<real><<<dim3(1, q.rows, 3), 128, 0, st>>>(q, Bv, Bv, 3);
+  }
   CK(cudaGetLastError());
   return GRPIC_OK;
 }
@@ -852,6 +925,7 @@ int grpic_fields_prepare(grpic_ctx* ctx, const grpic_field_state* s, grpic_vec3*
 int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3* B_n, const grpic_current* J_prev,
                          const grpic_current* J, double dt, void* stream) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   if (!s || !vec3_ok(&s->B_prev) || !vec3_ok(&s->B) || !vec3_ok(&s->D_prev) || !vec3_ok(&s->D) || !vec3_ok(B_n))
     return fail(ctx, GRPIC_EINVAL, "a field pointer is NULL");
   if ((J == nullptr) != (J_prev == nullptr)) return fail(ctx, GRPIC_EINVAL, "J and J_prev must both be given or both be NULL");
@@ -904,6 +978,7 @@ int grpic_fields_advance(grpic_ctx* ctx, grpic_field_state* s, const grpic_vec3*
 int grpic_step_host(grpic_ctx* ctx, grpic_particles* ph, const grpic_fields* fh, grpic_current* Jh, double dt,
                     int64_t* h2d_bytes, int64_t* d2h_bytes) {
   if (!ctx) return GRPIC_EINVAL;
+  if (int rd = check_device(ctx)) return rd;
   int rc = check_particles(ctx, ph, 0);
   if (rc) return rc;
   const bool want_prev = ph->i1_prev && ph->i2_prev && ph->dx1_prev && ph->dx2_prev;   // all four or none come back

@@ -179,8 +179,9 @@ __global__ void __launch_bounds__(128) k_ampere(const FieldGeom q, const V3<T> D
 // horizon: rows i1 in [-ng, n_const] take the values of row n_const + 1.  One thread per (row, column); component
 // c = blockIdx.z in the order D1 D2 D3 B1 B2 B3.
 template <typename T>
-__global__ void __launch_bounds__(128) k_field_bc_axis(const FieldGeom q, const V3<T> D, const V3<T> B) {
-  const int c = blockIdx.z, a1 = blockIdx.y, t = threadIdx.x + blockIdx.x * blockDim.x;
+__global__ void __launch_bounds__(128) k_field_bc_axis(const FieldGeom q, const V3<T> D, const V3<T> B, int c0) {
+  // c0 = 0 with gridDim.z = 6: all six components; c0 = 3 with gridDim.z = 3: B only (D is not touched)
+  const int c = blockIdx.z + c0, a1 = blockIdx.y, t = threadIdx.x + blockIdx.x * blockDim.x;
   if (t >= 2 * q.ng + 2) return;
   T* A = c < 3 ? D.f[c] : B.f[c - 3];
   const bool half = (c == 1 || c == 3 || c == 5);            // sampled at j + 1/2

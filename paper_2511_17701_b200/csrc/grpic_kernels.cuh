@@ -174,12 +174,23 @@ __global__ void __launch_bounds__(kBlock) k_push_or_step(const Consts<T> g, cons
   particle_direct<T, kDeposit, CoordT>(g, P, F, J, sc, counters, k);
 }
 
+// The same over the slots [*first_ptr, P.n) with *first_ptr read on the device: the slots behind the alive particles of
+// the last sort (dead then, possibly revived or appended since), which the tile table does not cover.  Fixed grid,
+// block-strided, so that the host never has to know the alive count (no read-back in grpic_sort).
+template <typename T, bool kDeposit, typename CoordT = Coord<T>>
+__global__ void __launch_bounds__(kBlock) k_push_or_step_from(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F,
+                                                              const JPtrs<T> J, const SpeciesConst sc,
+                                                              unsigned long long* counters, const uint32_t* first_ptr) {
+  const int64_t first = (int64_t)first_ptr[0];
+  for (int64_t base = first + (int64_t)blockIdx.x * kBlock; base < P.n; base += (int64_t)gridDim.x * kBlock)
+    particle_direct<T, kDeposit, CoordT>(g, P, F, J, sc, counters, base + threadIdx.x);
+}
+
 // deposit from stored (prev, current) — Eq. 36 velocity recomputed at the path midpoint as the paper
 // states it
 template <typename T, typename CoordT = Coord<T>>
-__global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J,
-                                                    const SpeciesConst sc, unsigned long long* counters) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+__device__ __forceinline__ void deposit_direct(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>& J,
+                                               const SpeciesConst& sc, unsigned long long* counters, int64_t k) {
   bool over = false;
   if (k < P.n && P.tag[k] != 0) {
     const int ia = P.i1p[k], ja = P.i2p[k];
@@ -200,6 +211,21 @@ __global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPt
     }
   }
   warp_count(counters, 3, over);
+}
+
+template <typename T, typename CoordT = Coord<T>>
+__global__ void __launch_bounds__(kBlock) k_deposit(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J,
+                                                    const SpeciesConst sc, unsigned long long* counters) {
+  deposit_direct<T, CoordT>(g, P, J, sc, counters, (int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+}
+// slots [*first_ptr, P.n), see k_push_or_step_from
+template <typename T, typename CoordT = Coord<T>>
+__global__ void __launch_bounds__(kBlock) k_deposit_from(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J,
+                                                         const SpeciesConst sc, unsigned long long* counters,
+                                                         const uint32_t* first_ptr) {
+  const int64_t first = (int64_t)first_ptr[0];
+  for (int64_t base = first + (int64_t)blockIdx.x * kBlock; base < P.n; base += (int64_t)gridDim.x * kBlock)
+    deposit_direct<T, CoordT>(g, P, J, sc, counters, base + threadIdx.x);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -307,7 +307,7 @@ template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 1))
     k_step_tiled(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr,
-                 uint32_t max_items, int64_t n_at_sort, int nt2, int use_tma, int skip_dense,
+                 int nt2, int use_tma, int skip_dense,
                  const __grid_constant__ FieldMaps maps) {
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the kWarps private J tiles
@@ -318,12 +318,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   T* sJ = sF + wid * kJTile;                          // this warp's private J tile
-  // ---- tail blocks: particles appended after the last sort -> direct path ----
-  if (blockIdx.x >= max_items) {
-    const int64_t k = n_at_sort + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
-    particle_direct<T, kDeposit, CoordT>(g, P, F, J, sc, counters, k);
-    return;
-  }
+  // (slots behind the alive particles of the last sort: k_push_or_step_from, launched beside this kernel)
   if (blockIdx.x >= n_items_ptr[0]) return;
   const WorkItem item = items[blockIdx.x];
   if (skip_dense && item.pad) return;                 // a dense item: k_step_lanes has it (grpic_lanes.cuh)
@@ -528,8 +523,7 @@ constexpr size_t deposit_smem_bytes() {
 template <typename T, typename CoordT = Coord<T>>
 __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 2))
     k_deposit_tiled(const Consts<T> g, const PPtrs<T> P, const JPtrs<T> J, const SpeciesConst sc,
-                    unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr, uint32_t max_items,
-                    int64_t n_covered, int nt2) {
+                    unsigned long long* counters, const WorkItem* items, const uint32_t* n_items_ptr, int nt2) {
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sF = reinterpret_cast<T*>(smem_raw_);
   T* sQv = sF + kJElems;
@@ -571,14 +565,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
     }
   };
 
-  if (blockIdx.x >= max_items) {                      // slots the table does not cover: straight to L2
-    const int64_t k = n_covered + (int64_t)(blockIdx.x - max_items) * kTBlock + tid;
-    bool da, db; int na, nb; T seg[2][8];
-    one(k, false, 0, 0, da, na, db, nb, seg);
-    if (n_over) atomicAdd(&counters[3], (unsigned long long)n_over);
-    return;
-  }
-  if (blockIdx.x >= n_items_ptr[0]) return;
+  if (blockIdx.x >= n_items_ptr[0]) return;         // (slots the table does not cover: k_deposit_from)
   const WorkItem item = items[blockIdx.x];
   const int c1lo = (int)(item.tile / (uint32_t)nt2) * kTile - kHalo;
   const int c2lo = (int)(item.tile % (uint32_t)nt2) * kTile - kHalo;
@@ -625,7 +612,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
 template <typename T, typename CoordT = Coord<T>>
 bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>& J, const SpeciesConst& sc,
                           unsigned long long* counters, const WorkItem* items, const uint32_t* d_n_items,
-                          uint32_t max_items, int64_t n_covered, bool& attr_set, cudaStream_t st, std::string& err) {
+                          uint32_t max_items, bool& attr_set, cudaStream_t st, std::string& err) {
   // attr_set: the shared-memory opt-in is per device and per loaded module; the flag lives in the context
   if (!attr_set) {
     cudaError_t ea = cudaFuncSetAttribute(k_deposit_tiled<T, CoordT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -637,10 +624,8 @@ bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>&
     attr_set = true;
   }
   const int nt2 = (g.n2 + kTile - 1) / kTile;
-  const int64_t tail = P.n > n_covered ? P.n - n_covered : 0;
-  const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
-  k_deposit_tiled<T, CoordT><<<grid, kTBlock, deposit_smem_bytes<T>(), st>>>(g, P, J, sc, counters, items, d_n_items,
-                                                                            max_items, n_covered, nt2);
+  k_deposit_tiled<T, CoordT><<<max_items, kTBlock, deposit_smem_bytes<T>(), st>>>(g, P, J, sc, counters, items,
+                                                                                 d_n_items, nt2);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     err = std::string("k_deposit_tiled launch: ") + cudaGetErrorString(e);
@@ -652,7 +637,7 @@ bool launch_deposit_tiled(const Consts<T>& g, const PPtrs<T>& P, const JPtrs<T>&
 template <typename T, typename CoordT = Coord<T>, bool kDeposit = true>
 bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g, const PPtrs<T>& P, const FPtrs<T>& F,
                        const JPtrs<T>& J, const SpeciesConst& sc, unsigned long long* counters,
-                       const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items, int64_t n_at_sort,
+                       const WorkItem* items, const uint32_t* d_n_items, uint32_t max_items,
                        bool skip_dense, bool& attr_set, cudaStream_t st, std::string& err) {
   if (!attr_set) {
     cudaError_t ea = cudaFuncSetAttribute(k_step_tiled<T, CoordT, kDeposit>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -670,10 +655,8 @@ bool launch_step_tiled(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   for (int c = 0; c < 6 && use_tma; ++c)
     if (!enc.encode(&maps.m[c], F.f[c], (int)sizeof(T), rows, g.ld)) use_tma = 0;
   const int nt2 = (g.n2 + kTile - 1) / kTile;
-  const int64_t tail = P.n > n_at_sort ? P.n - n_at_sort : 0;
-  const unsigned grid = max_items + (unsigned)((tail + kTBlock - 1) / kTBlock);
-  k_step_tiled<T, CoordT, kDeposit><<<grid, kTBlock, tiled_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, d_n_items, max_items,
-                                                                n_at_sort, nt2, use_tma, skip_dense ? 1 : 0, maps);
+  k_step_tiled<T, CoordT, kDeposit><<<max_items, kTBlock, tiled_smem_bytes<T>(), st>>>(
+      g, P, F, J, sc, counters, items, d_n_items, nt2, use_tma, skip_dense ? 1 : 0, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     err = std::string("k_step_tiled launch: ") + cudaGetErrorString(e);

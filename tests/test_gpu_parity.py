@@ -643,6 +643,9 @@ def test_full_pic_cycle_against_the_oracle(G, O, W, prec):
     for step in range(4):
         ctx.fields_prepare(sg, Bn_g, dt)
         Bn_o = O.fields_prepare(g, so, dt)
+        for k in kb:                                   # (n)B itself, ghost columns beyond the axes included
+            d = np.abs(Bn_g[k].cpu().numpy().astype(np.float64) - Bn_o[k]).max() / np.abs(Bn_o[k]).max()
+            assert d < (1e-5 if prec == "f32" else 1e-12), (step, k, d)
         Jg, Jo = zeros(kj), {k: np.zeros(g.shape) for k in kj}
         for ps, op in zip(sets, ops):
             ctx.step(ps, {**sg["D"], **Bn_g}, Jg, dt)

@@ -194,6 +194,28 @@ def test_field_bc_leaves_an_axisymmetric_solution_unchanged(O, W):
             assert np.array_equal(r[k][row], r[k][G + 3])                                           # layer = row n_f + 1
 
 
+def test_prepared_B_has_axis_ghosts_of_its_own_time_level(O):
+    """(n)B of fields_prepare (Eq. 46-48) is what the particle gather reads, ghost columns included.  With a field that
+    changes in time ((n-3/2)B != (n-1/2)B, D != 0) the ghost columns beyond the axes must be the mirror images of
+    the PHYSICAL columns of (n)B itself - not left at the averaged level n-1, which Faraday does not update."""
+    g = O.Grid(24, 16, 0.8, 1.5, 12.0)
+    rng = np.random.default_rng(11)
+    mk = lambda ks: {k: rng.normal(size=g.shape) for k in ks}
+    st = dict(B_prev=mk(("B1", "B2", "B3")), B=mk(("B1", "B2", "B3")), D_prev=mk(("D1", "D2", "D3")), D=mk(("D1", "D2", "D3")))
+    for name in st:
+        O.field_bc(g, st[name])                       # the state itself obeys the axis symmetry
+    Bn = O.fields_prepare(g, st, 0.05)
+    G, n2 = g.ng, g.n2
+    avg = {k: 0.5 * (st["B_prev"][k] + st["B"][k]) for k in Bn}
+    assert max(np.abs(Bn[k] - avg[k])[G + 1:-G - 1, G + 1:G + n2 - 1].max() for k in Bn) > 1e-3      # Faraday did act
+    for m in range(1, G + 1):
+        assert np.array_equal(Bn["B1"][:, G - m], Bn["B1"][:, G + m - 1])                # even, sampled at j + 1/2
+        assert np.array_equal(Bn["B1"][:, G + n2 + m - 1], Bn["B1"][:, G + n2 - m])
+        assert np.array_equal(Bn["B3"][:, G - m], Bn["B3"][:, G + m - 1])
+        assert np.array_equal(Bn["B2"][:, G - m], -Bn["B2"][:, G + m])                   # odd, sampled at j
+    assert not Bn["B2"][:, G].any() and not Bn["B2"][:, G + n2].any()
+
+
 def test_current_filter_properties(O):
     """Binomial filter (reading R-F5): constants are invariant, the Nyquist mode along x1 is annihilated in one pass,
     n passes along x1 are the convolution with the binomial coefficients C(2n, k)/4^n, the filter commutes with the
