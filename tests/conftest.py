@@ -24,3 +24,31 @@ def O():
 def W():
     from paper_2511_17701_b200 import workloads
     return workloads
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Evidence for the two FP32 allowances of the parity rules, printed with every GPU run."""
+    try:
+        import helpers
+        rows = helpers.AXIS_STATS
+    except Exception:
+        return
+    if not rows:
+        return
+    tr = terminalreporter
+    for prec in ("f32", "f64"):
+        r = [x for x in rows if x[0] == prec]
+        if not r:
+            continue
+        n_ax = sum(x[2] for x in r)
+        tr.write_line(f"[parity] {prec}: {len(r)} particle comparisons, {sum(x[1] for x in r)} particles; "
+                      f"axis allowance (kappa > 1) used by {n_ax} particles in {sum(1 for x in r if x[2])} comparisons, "
+                      f"their max raw error {max(x[3] for x in r):.2e} (tolerance {helpers.TOL[prec]['x']:.0e}), max kappa {max(x[4] for x in r):.1f}")
+    try:
+        import test_gpu_parity as t
+        s = t.STRADDLE_STEPS
+        tr.write_line(f"[parity] steps whose J comparison substituted face-straddling particles: {len(s)} "
+                      f"({sum(n for _, n in s)} particles; by precision: " +
+                      ", ".join(f"{p} {sum(1 for q, _ in s if q == p)}" for p in ("f32", "f64")) + ")")
+    except Exception:
+        pass

@@ -91,6 +91,7 @@ def oracle_particles(O, sp, dtype=np.float64):
 # GPU-vs-oracle parity helpers (north_star tolerances made operational)
 # --------------------------------------------------------------------------------------------
 TOL = {"f64": dict(x=1e-12, u=1e-12, J=1e-10), "f32": dict(x=1e-5, u=1e-5, J=1e-5)}
+AXIS_STATS = []      # one row per compare_particles call: (precision, particles, n with kappa > 1, their max raw error, max kappa)
 
 
 def oracle_from_cols(O, cols, q_over_m, charge, massive):
@@ -139,7 +140,13 @@ def compare_particles(op, gc, prec, was_alive, n1, n2, check_prev=True, diag=Non
     mid2 = p2 + 0.5 * del2
     d_axis = np.maximum(np.minimum(mid2, n2 - mid2), 1e-5 / (np.pi / n2))
     kappa = np.maximum(1.0, 0.5 * np.abs(del2) / d_axis)
-    out["n_axis"] = int((kappa[m] > 1.0).sum())
+    if prec == "f64":
+        kappa = np.ones_like(kappa)                   # FP64 meets the flat north_star bound everywhere: no allowance
+    ax = (kappa > 1.0) & m
+    out["n_axis"] = int(ax.sum())
+    out["axis_raw"] = float((ex / xn)[ax].max(initial=0.0))      # their largest error WITHOUT the allowance
+    out["k_max"] = float(kappa[m].max(initial=1.0))
+    AXIS_STATS.append((prec, int(m.sum()), out["n_axis"], out["axis_raw"], out["k_max"]))
     ex = (ex / (xn * kappa))[m]
     out["x_err"] = float(ex.max(initial=0.0))
     du = np.max(np.abs(np.stack([f("u1") - op.u1, f("u2") - op.u2, f("u3") - op.u3])), axis=0)[m]
@@ -162,6 +169,16 @@ def compare_particles(op, gc, prec, was_alive, n1, n2, check_prev=True, diag=Non
     ok = ~(bad_idx[m])
     assert np.all(ex[ok] <= tx), f"position error {out['x_err']:.3e} > {tx}"
     assert np.all(eu[ok] <= tol["u"]), f"momentum error {out['u_err']:.3e} > {tol['u']}"
+    # absolute bounds in cell units / radians (the norm-wise rule above is loose at i1 ~ 2000): measured 2e-7 (f32)
+    abs_tol = 2e-6 if prec == "f32" else 1e-11
+    plain = m & ~((kappa > 1.0))
+    dxa = np.max(np.abs(np.stack([gx1 - ox1, gx2 - ox2])), axis=0)
+    assert np.all(dxa[plain] <= abs_tol), f"in-cell position error {dxa[plain].max():.3e} cells > {abs_tol}"
+    dph = np.abs(gphi - ophi)
+    assert np.all(dph[plain] <= abs_tol * np.maximum(1.0, np.abs(ophi[plain]))), f"phi error {dph[plain].max():.3e}"
+    # the axis allowance: a handful of FP32 particles, their raw error bounded absolutely as well
+    assert out["n_axis"] <= max(4, 2e-4 * m.sum()), f"{out['n_axis']} particles lean on the axis-conditioning allowance"
+    assert out["axis_raw"] <= 5e-5, f"raw error of an axis-grazing particle {out['axis_raw']:.3e}"
     # dead-before particles are untouched
     d = ~m
     for k in ("i1", "i2", "dx1", "dx2", "u1", "u2", "u3", "tag"):

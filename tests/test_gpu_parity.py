@@ -59,14 +59,31 @@ def _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode, sort_first=F
         c = ctx.counters()
     diag = {}
     alive, a_in, a_out = O.push(g, op, fhost if ps.q_over_m != 0 and ps.massive else None, dt, diag=diag)
-    Jo, over = O.deposit(g, op, dt)
     after = ps.to_numpy()
     res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag,
                             check_prev=before["i1_prev"] is not None)
-    if res["n_idx_mismatch"] == 0:
-        assert (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"]) == (alive, a_in, a_out, over), (c, alive, a_in, a_out, over)
-        res.update(compare_current(Jo, _J_np(J), prec))
+    if res["n_idx_mismatch"]:
+        # FP32 only (compare_particles asserts 0 for f64): a particle within rounding of a cell face ended in the
+        # neighbouring cell (or, at a radial edge, on the other side of the absorption test).  J is still compared,
+        # entry by entry: the oracle deposits those few particles from the GPU's (cell, displacement, tag) - the same
+        # continuous position within tolerance, as compare_particles has just checked - and all others from its own.
+        bad = np.flatnonzero(((after["i1"] != op.i1) | (after["i2"] != op.i2) | (after["tag"] != op.tag)) & (before["tag"] != 0))
+        for k in ("i1", "i2", "dx1", "dx2", "tag"):
+            getattr(op, k)[bad] = after[k][bad]
+        STRADDLE_STEPS.append((prec, len(bad)))
+        alive = int(op.tag[before["tag"] != 0].sum())
+        a_in = a_out = None
+    Jo, over = O.deposit(g, op, dt)
+    exp = (alive, a_in, a_out, over)
+    got = (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"])
+    assert all(e is None or e == v for e, v in zip(exp, got)), (c, exp)
+    if a_in is None:
+        assert c["absorbed_in"] + c["absorbed_out"] == int((before["tag"] != 0).sum()) - alive
+    res.update(compare_current(Jo, _J_np(J), prec))
     return res, c
+
+
+STRADDLE_STEPS = []      # (precision, particles) of every step whose J comparison went through the substitution above
 
 
 @pytest.mark.parametrize("mode", ["split", "fused"])
@@ -208,10 +225,14 @@ def test_general_a3_map(G, O, W, prec, r0, h0, lin, mass):
     fields = {k: 0.3 * np.sin(0.21 * ii + p) * np.cos(0.17 * jj - p) + 0.05 * rng.uniform(-1, 1, shape)
               for p, k in enumerate(("D1", "D2", "D3", "B1", "B2", "B3"))}
     n = 40000
-    # two rows of cells next to each axis stay empty: a lone particle a few 1e-4 cells from the axis owns max|J3| there
-    # (v^3 ~ 1/sin^2 theta) and its FP32 conditioning, not the kernel, would set the J3 error of this small case
-    i1 = rng.integers(0, n1, n).astype(np.int32); i2 = rng.integers(2, n2 - 2, n).astype(np.int32)
+    # particles in every cell, the two rows next to the axes included: they reflect through the general map.
+    # FP64: anywhere in the cell.  FP32: a lone particle a few 1e-4 cells from the axis owns max|J3| of this small case
+    # (v^3 ~ 1/sin^2 theta) and the FP32 conditioning of 1/sin^2 at that angle, not the kernel, would set the J3 error,
+    # so FP32 starts at least 0.1 cell from an axis (reflections still happen: paths of up to 0.4 cell per step).
+    i1 = rng.integers(0, n1, n).astype(np.int32); i2 = rng.integers(0, n2, n).astype(np.int32)
     dx1, dx2 = rng.random(n), rng.random(n)
+    if prec == "f32":
+        dx2 = np.where(i2 == 0, np.maximum(dx2, 0.1), np.where(i2 == n2 - 1, np.minimum(dx2, 0.9), dx2))
     m = O.metric(g, i1 + dx1, i2 + dx2, derivs=False)
     uh = rng.uniform(-0.7, 0.7, (3, n))                       # roughly orthonormal-frame sized momenta
     cells = O.metric(g, *[v.ravel() for v in np.meshgrid(np.arange(n1) + 0.5, np.arange(n2) + 0.5, indexing="ij")], derivs=False)
