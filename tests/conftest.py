@@ -45,8 +45,7 @@ def pytest_terminal_summary(terminalreporter):
                       f"axis allowance (kappa > 1) used by {n_ax} particles in {sum(1 for x in r if x[2])} comparisons, "
                       f"their max raw error {max(x[3] for x in r):.2e} (tolerance {helpers.TOL[prec]['x']:.0e}), max kappa {max(x[4] for x in r):.1f}")
     try:
-        import test_gpu_parity as t
-        s = t.STRADDLE_STEPS
+        s = helpers.STRADDLE_STEPS
         tr.write_line(f"[parity] steps whose J comparison substituted face-straddling particles: {len(s)} "
                       f"({sum(n for _, n in s)} particles; by precision: " +
                       ", ".join(f"{p} {sum(1 for q, _ in s if q == p)}" for p in ("f32", "f64")) + ")")

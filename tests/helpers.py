@@ -189,6 +189,24 @@ def compare_particles(op, gc, prec, was_alive, n1, n2, check_prev=True, diag=Non
     return out
 
 
+STRADDLE_STEPS = []      # (precision, particles) of every step whose J comparison went through the substitution below
+
+
+def oracle_deposit_as_the_gpu_decided(O, g, op, after, was_alive, dt, prec):
+    """Oracle deposit of the pushed oracle particles `op`, entry-by-entry comparable with the GPU's J even when a few
+    FP32 particles within rounding of a cell face ended in the neighbouring cell (or, at a radial edge, on the other
+    side of the absorption test): those particles - compare_particles has checked that their continuous position
+    agrees within tolerance, and asserts that FP64 has none - are deposited from the GPU's (cell, displacement, tag).
+    Returns (J, n_overstep, n_substituted)."""
+    bad = np.flatnonzero(((after["i1"] != op.i1) | (after["i2"] != op.i2) | (after["tag"] != op.tag)) & (was_alive != 0))
+    if len(bad):
+        for k in ("i1", "i2", "dx1", "dx2", "tag"):
+            getattr(op, k)[bad] = after[k][bad]
+        STRADDLE_STEPS.append((prec, len(bad)))
+    Jo, over = O.deposit(g, op, dt)
+    return Jo, over, len(bad)
+
+
 def compare_current(Jo, Jg, prec):
     tol = TOL[prec]["J"]
     out = {}

@@ -6,7 +6,8 @@ first moments, conserved u_3 and energy of geodesics)."""
 import numpy as np
 import pytest
 
-from helpers import TOL, compare_particles, grid_from_domain, oracle_from_cols
+from helpers import (TOL, compare_current, compare_particles, grid_from_domain, oracle_deposit_as_the_gpu_decided,
+                     oracle_from_cols)
 
 pytestmark = pytest.mark.gpu
 
@@ -131,6 +132,54 @@ def test_configs_3_4_5_full_size(G, O, W, name, prec, tol_cont, tol_mom):
     e2 = abs(float(J2.sum()) - m2) / scale_sp
     print(name, "full: first-moment errors", e1, e2)
     assert e1 < tol_mom and e2 < tol_mom
+
+
+@pytest.mark.parametrize("name,prec", [("large", "f32"), ("two_species", "f64")])
+def test_full_size_every_particle_and_every_J_entry(G, O, W, name, prec):
+    """Element-wise parity at full size in the launch configuration bench.py times: one species of config 4
+    (2048x1024, 67 M electrons, FP32) and of config 5 (1024x1024, 33.5 M electrons, FP64) - two column sets without
+    *_prev, grpic_sort_into with sort_lookahead = 5, three steps of drift, then ONE fused grpic_step whose result is
+    compared with the oracle run on ALL particles of the species: every particle (compare_particles) and every entry
+    of J^1, J^2, J^3 (Eq. 34, 36) at 1e-5 max|J| (FP32) / 1e-10 max|J| (FP64)."""
+    import torch
+    wl = dict(large=W.config_large, two_species=W.config_two_species)[name]()
+    dom = wl.dom
+    g = grid_from_domain(O, dom)
+    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
+    names = ("D1", "D2", "D3", "B1", "B2", "B3")
+    fdev = G.grid_tensors(wl.fields, names, prec)
+    fhost = {k: fdev[k].cpu().numpy().astype(np.float64) for k in names}
+    J = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
+    sp = wl.species[0]
+    src = G.ParticleSet.from_host(sp, prec).drop_prev()
+    ps = src.empty_like()
+    ctx.sort_into(src, ps)                                # first sort: present-cell key (no dt yet)
+    ctx.set_real("sort_lookahead", 5.0)
+    for _ in range(2):
+        ctx.step(ps, fdev, J, wl.dt)
+    ctx.sort_into(ps, src)                                # look-ahead sort, as in bench.py's steady state
+    ps = src
+    for _ in range(3):                                    # drift away from the sorted order
+        ctx.step(ps, fdev, J, wl.dt)
+    for v in J.values():
+        v.zero_()
+    before = ps.to_numpy()
+    ctx.step(ps, fdev, J, wl.dt)
+    c = ctx.counters()
+    after = ps.to_numpy()
+    Jg = {k: v.cpu().numpy().astype(np.float64) for k, v in J.items()}
+    del ps, src, J
+    torch.cuda.empty_cache()
+    op = oracle_from_cols(O, before, sp.q_over_m, sp.charge, sp.massive)
+    diag = {}
+    alive, a_in, a_out = O.push(g, op, fhost, wl.dt, diag=diag)
+    res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag, check_prev=False)
+    Jo, over, n_sub = oracle_deposit_as_the_gpu_decided(O, g, op, after, before["tag"], wl.dt, prec)
+    if n_sub == 0:
+        assert (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"]) == (alive, a_in, a_out, over)
+    res.update(compare_current(Jo, Jg, prec))
+    print(name, "full, all particles:", res, c, "substituted", n_sub)
+    assert c["alive"] > 0.9 * int((before["tag"] != 0).sum()) and c["absorbed_in"] > 0
 
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])

@@ -5,7 +5,8 @@ Every case runs the library through paper_2511_17701_b200.grpic (ctypes -> libgr
 import numpy as np
 import pytest
 
-from helpers import TOL, compare_current, compare_particles, grid_from_domain, oracle_from_cols
+from helpers import (TOL, compare_current, compare_particles, grid_from_domain, oracle_deposit_as_the_gpu_decided,
+                     oracle_from_cols)
 
 pytestmark = pytest.mark.gpu
 
@@ -62,28 +63,15 @@ def _one_step_parity(G, O, ctx, g, ps, fdev, fhost, dt, prec, mode, sort_first=F
     after = ps.to_numpy()
     res = compare_particles(op, after, prec, before["tag"], g.n1, g.n2, diag=diag,
                             check_prev=before["i1_prev"] is not None)
-    if res["n_idx_mismatch"]:
-        # FP32 only (compare_particles asserts 0 for f64): a particle within rounding of a cell face ended in the
-        # neighbouring cell (or, at a radial edge, on the other side of the absorption test).  J is still compared,
-        # entry by entry: the oracle deposits those few particles from the GPU's (cell, displacement, tag) - the same
-        # continuous position within tolerance, as compare_particles has just checked - and all others from its own.
-        bad = np.flatnonzero(((after["i1"] != op.i1) | (after["i2"] != op.i2) | (after["tag"] != op.tag)) & (before["tag"] != 0))
-        for k in ("i1", "i2", "dx1", "dx2", "tag"):
-            getattr(op, k)[bad] = after[k][bad]
-        STRADDLE_STEPS.append((prec, len(bad)))
-        alive = int(op.tag[before["tag"] != 0].sum())
-        a_in = a_out = None
-    Jo, over = O.deposit(g, op, dt)
+    Jo, over, n_sub = oracle_deposit_as_the_gpu_decided(O, g, op, after, before["tag"], dt, prec)
+    if n_sub:                                          # a face-straddler may have been absorbed on one side only
+        alive, a_in, a_out = int(op.tag[before["tag"] != 0].sum()), None, None
+        assert c["absorbed_in"] + c["absorbed_out"] == int((before["tag"] != 0).sum()) - alive
     exp = (alive, a_in, a_out, over)
     got = (c["alive"], c["absorbed_in"], c["absorbed_out"], c["overstep"])
     assert all(e is None or e == v for e, v in zip(exp, got)), (c, exp)
-    if a_in is None:
-        assert c["absorbed_in"] + c["absorbed_out"] == int((before["tag"] != 0).sum()) - alive
     res.update(compare_current(Jo, _J_np(J), prec))
     return res, c
-
-
-STRADDLE_STEPS = []      # (precision, particles) of every step whose J comparison went through the substitution above
 
 
 @pytest.mark.parametrize("mode", ["split", "fused"])
