@@ -35,7 +35,9 @@
  *                  inside one cell and for one across a face).
  */
 #define _USE_MATH_DEFINES
+#ifndef _GNU_SOURCE
 #define _GNU_SOURCE
+#endif
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -43,6 +45,17 @@
 #ifdef _OPENMP
 #include <omp.h>
 #endif
+
+/* Operation count of this statement of the method: the same source compiled as C++ with -DORC_COUNT
+ * runs on a counting stand-in for `double` (oracle/orc_count.hpp); ORC_STAGE marks the stage the operations that
+ * follow belong to.  In the normal build the marks vanish and nothing else changes. */
+#ifdef ORC_COUNT
+#include "orc_count.hpp"
+#define double orc_cnt
+#else
+#define ORC_STAGE(s) ((void)0)
+#endif
+enum { ORC_ST_INTERP = 0, ORC_ST_METRIC, ORC_ST_EM, ORC_ST_ULOOP, ORC_ST_XLOOP, ORC_ST_BC, ORC_ST_DEPOSIT, ORC_ST_OTHER };
 
 typedef struct {
   int32_t n1, n2, ng;    /* N_r, N_theta, ghost width          */
@@ -327,10 +340,12 @@ static int orc_push_core(const orc_grid* g, orc_particles* p, int64_t k, const d
   const double x2n = (double)p->i2[k] + p->dx2[k];
   double u[3] = {p->u1[k], p->u2[k], p->u3[k]};
 
+  ORC_STAGE(ORC_ST_METRIC);
   orc_metric_t m; orc_dmetric_t d;
   orc_metric(g, x1n, x2n, &m);
   orc_dmetric(g, &m, &d);
 
+  ORC_STAGE(ORC_ST_EM);
   double Dh[3] = {0, 0, 0}, Bh[3] = {0, 0, 0}, uh[3];
   const double c = p->q_over_m * m.alpha * dt * 0.25;
   if (em) {
@@ -340,16 +355,20 @@ static int orc_push_core(const orc_grid* g, orc_particles* p, int64_t k, const d
     orc_boris_half(Dh, Bh, c, uh);                             /* 4 */
     orc_tetrad_to_cov(&m, uh, u);                              /* 5 */
   }
+  ORC_STAGE(ORC_ST_ULOOP);
   orc_geodesic_u(&m, &d, eps, dt, g->n_iter, u);               /* 6 */
+  ORC_STAGE(ORC_ST_EM);
   if (em) {
     orc_cov_to_tetrad(&m, u, uh);                              /* 7 */
     orc_boris_half(Dh, Bh, c, uh);                             /* 8 */
     orc_tetrad_to_cov(&m, uh, u);                              /* 9 */
   }
+  ORC_STAGE(ORC_ST_XLOOP);
   double del[2];
   const double dphidt = orc_geodesic_x(g, x1n, x2n, u, eps, dt, del);   /* 10 */
   if (orc_diag_del1) { orc_diag_del1[k] = del[0]; orc_diag_del2[k] = del[1]; }
   if (p->phi) p->phi[k] += dt * dphidt;                        /* 11 */
+  ORC_STAGE(ORC_ST_BC);
 
   /* renormalise to (cell, displacement in [0,1)) */
   int32_t i1 = p->i1[k], i2 = p->i2[k];
@@ -382,6 +401,7 @@ void orc_push(const orc_grid* g, orc_particles* p, const orc_fields* F, double d
   for (int64_t k = 0; k < p->n; ++k) {
     if (!p->tag[k]) continue;
     double Dp[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
+    ORC_STAGE(ORC_ST_INTERP);
     if (em) orc_interp(g, F, p->i1[k], p->i2[k], p->dx1[k], p->dx2[k], Dp, Bp);   /* 2 */
     const int r = orc_push_core(g, p, k, Dp, Bp, dt);
     c0 += (r == 0); c1 += (r == 1); c2 += (r == 2);
@@ -412,6 +432,7 @@ typedef struct { double *J1, *J2, *J3; } orc_current;
 
 static void orc_deposit_one(const orc_grid* g, const orc_particles* p, int64_t k, double dt,
                             double* J1, double* J2, double* J3, int64_t* overstep) {
+  ORC_STAGE(ORC_ST_DEPOSIT);
   const int64_t ld = g->n2 + 2 * g->ng;
   const int ia = p->i1_prev[k], ja = p->i2_prev[k], ib = p->i1[k], jb = p->i2[k];
   const int di = ib - ia, dj = jb - ja;
@@ -681,3 +702,29 @@ void orc_ampere(const orc_grid* g, double* D1, double* D2, double* D3, const dou
     }
   }
 }
+
+#ifdef ORC_COUNT
+/* One push + deposit of every alive particle on the counting type, single thread; out[stage][kind] receives the
+ * totals (layout ORC_N_STAGES x ORC_N_KINDS of orc_count.hpp), *n_particles the number of particles counted. */
+extern "C" void orc_count_step(const orc_grid* g, orc_particles* p, const orc_fields* F, orc_current* J, const double* dt,
+                               int64_t* out, int64_t* n_particles) {
+  for (int s = 0; s < ORC_N_STAGES; ++s)
+    for (int k = 0; k < ORC_N_KINDS; ++k) orc_counts[s][k] = 0;
+  const int em = (p->q_over_m != 0.0) && p->massive;
+  int64_t n = 0, over = 0;
+  ORC_STAGE(ORC_ST_OTHER);
+  for (int64_t k = 0; k < p->n; ++k) {
+    if (!p->tag[k]) continue;
+    ++n;
+    double Dp[3] = {0, 0, 0}, Bp[3] = {0, 0, 0};
+    ORC_STAGE(ORC_ST_INTERP);
+    if (em) orc_interp(g, F, p->i1[k], p->i2[k], p->dx1[k], p->dx2[k], Dp, Bp);
+    orc_push_core(g, p, k, Dp, Bp, *dt);
+    if (p->tag[k] && p->charge != 0.0) orc_deposit_one(g, p, k, *dt, J->J1, J->J2, J->J3, &over);
+    ORC_STAGE(ORC_ST_OTHER);
+  }
+  for (int s = 0; s < ORC_N_STAGES; ++s)
+    for (int k = 0; k < ORC_N_KINDS; ++k) out[s * ORC_N_KINDS + k] = orc_counts[s][k];
+  *n_particles = n;
+}
+#endif

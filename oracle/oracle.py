@@ -33,6 +33,46 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_LIB_COUNT = os.path.join(_HERE, "libgrpic_oracle_count.so")
+COUNT_STAGES = ("interpolation (S4)", "metric + 12 derivatives at x^n (S1, S2)", "tetrad projections + 2 Boris halves (S3, S5)",
+                "momentum loop Eq. 26-27 (S6)", "coordinate loop Eq. 28-29 + phi Eq. 30 (S7, S8)",
+                "renormalise + particle BCs (S9)", "deposit incl. v^3 at the path midpoint (S10)", "other")
+COUNT_KINDS = ("add/sub", "mul", "div", "sqrt", "exp/log", "sin/cos", "floor", "min/max", "compare", "neg/abs")
+
+
+def build_count(force: bool = False) -> str:
+    """The same C source compiled as C++ on the operation-counting stand-in for double (oracle/orc_count.hpp)."""
+    deps = [_SRC, os.path.join(_HERE, "orc_count.hpp")]
+    if force or not os.path.exists(_LIB_COUNT) or any(os.path.getmtime(_LIB_COUNT) < os.path.getmtime(d) for d in deps):
+        cmd = ["g++", "-x", "c++", "-O1", "-std=gnu++17", "-ffp-contract=off", "-DORC_COUNT", "-shared", "-fPIC", _SRC,
+               "-o", _LIB_COUNT, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB_COUNT
+
+
+def count_ops(g: "Grid", p: "Particles", fields, dt: float) -> dict:
+    """Operations the oracle, as written, executes for one push + deposit of the alive particles of a COPY of `p`:
+    {"per_update": {stage: {kind: count per particle}}, "total_per_update": float, "particles": n}.
+    Every +, -, *, /, sqrt, exp, log, sin, cos, floor, fmin/fmax, comparison and negation on a real number counts 1."""
+    L = C.CDLL(build_count())
+    q = p.copy()
+    gc = g.c(); pc = q.c()
+    J = {k: np.zeros(g.shape) for k in ("J1", "J2", "J3")}
+    jc = _Current(*[_ptr(J[k], _dp) for k in ("J1", "J2", "J3")])
+    out = np.zeros((len(COUNT_STAGES), len(COUNT_KINDS)), np.int64)
+    n = C.c_int64(0)
+    dtc = C.c_double(dt)
+    if fields is None:
+        L.orc_count_step(C.byref(gc), C.byref(pc), None, C.byref(jc), C.byref(dtc), out.ctypes.data_as(C.c_void_p), C.byref(n))
+    else:
+        fc, keep = _fields_c(fields)
+        L.orc_count_step(C.byref(gc), C.byref(pc), C.byref(fc), C.byref(jc), C.byref(dtc), out.ctypes.data_as(C.c_void_p), C.byref(n))
+    npart = max(1, int(n.value))
+    per = {st: {kd: out[i, j] / npart for j, kd in enumerate(COUNT_KINDS)} for i, st in enumerate(COUNT_STAGES)}
+    return {"per_update": per, "per_stage": {st: float(out[i].sum()) / npart for i, st in enumerate(COUNT_STAGES)},
+            "total_per_update": float(out.sum()) / npart, "particles": int(n.value), "n_iter": g.n_iter}
+
+
 class _Grid(C.Structure):
     _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("ng", C.c_int32), ("n_iter", C.c_int32),
                 ("a", C.c_double), ("r_min", C.c_double), ("r_max", C.c_double), ("small_angle", C.c_double),
