@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — particle updates/s of the GRPIC per-particle hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large|...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload large|...] [--peaks]
 
 A "step" = one pass of the whole hot path (interp + GR push + BCs + deposit, both species; the counting sort
 every `sort_every` steps as config 4 says: grpic_sort_into between two column sets, key of the cell predicted
@@ -11,12 +11,17 @@ FP32, sort every 10 steps) — the >= 100M-particle configuration north_star's t
 N > 1: the path does not shard (replicas only) -> every rank runs an independent
 replica of the same workload (seed + rank), weak scaling, no data-path collective.
 
+The line carries, besides the contract's keys: `roofline` (ALU-bound: algorithmic and executed fractions of the FMA
+peak MEASURED in this run by register-only FFMA/DFMA chains, and the HBM fraction), `other_workloads` (configs 3 and 5,
+the latter in FP64), `cpu_baseline` (the oracle on one FULL step of the workload on the host cores) and `e2e`.
+
 --impl reference times the oracle (oracle/, plain FP64 C, as it stands) on the host cores on a bounded
-sample of the same workload; rank 0 only.
+sample of the same workload; rank 0 only.   --peaks prints the measured throughput denominators and exits.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -32,29 +37,35 @@ sys.path.insert(0, ROOT)
 METRIC = "particle updates/sec (interp+GR push+deposit)"
 UNIT = "updates/s"
 
-# Algorithmic figures per particle update: what the method, as the paper states
-# it with n_iter = 10, must compute and move.
-FLOPS_PER_UPDATE_NITER10 = 2051.0          # DESIGN.md section 7 table: +,-,*,/,sqrt,exp,sin,cos,floor,min,max,compare each count 1
+# Algorithmic figures per particle update: what the method, as the paper states it with
+# n_iter = 10, must compute and move.  2051 = hand table with common sub-expressions shared and unused metric entries
+# dropped; the oracle AS WRITTEN executes ~3160 (counted by code: oracle.count_ops, reported in cpu_baseline).
+FLOPS_PER_UPDATE_NITER10 = 2051.0
 BYTES_PER_UPDATE = {"f32": 70.0, "f64": 122.0}   # fused step: read i,dx,u,phi,w,tag; write i,dx,u,phi,tag
-# FP32 FMA peak from unit counts and clocks (B200_PROFILING.md: 148 SMs, 1965 MHz; 128 FP32 lanes/SM, FMA = 2)
-ALU_PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+# FMA peak from unit counts and clocks (B200_PROFILING.md: 148 SMs, 1965 MHz; 128 FP32 / 64 FP64 lanes per SM, FMA = 2):
+# kept beside the measured figure for comparison
+ALU_PEAK_DERIVED = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
+KERNELS_PER_STEP_CALL = 3       # k_step_tiled (sparse items) + k_step_lanes (dense items) + k_push_or_step_from (tail)
+KERNELS_PER_SORT = 11           # hist, 3 x scan, items_count, 3 x scan, items_fill, rank, gather
 
 
-def _ncu_traffic(prec, workload):
-    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-    (profiles/ncu_traffic.csv: kernel,precision,workload,particles,dram_read_bytes,dram_write_bytes,source)."""
+def _profile_numbers(prec, workload):
+    """Per-launch numbers of the dominant kernel from the committed `ncu --set full` extract of this workload
+    (profiles/r2_top_kernel_<prec>_<workload>.csv, written from `ncu --page raw --csv` by the command named in the .md
+    beside it): DRAM bytes and executed FP instructions."""
+    path = os.path.join(ROOT, "profiles", f"r2_top_kernel_{prec}_{workload}.csv")
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
-            for line in f:
-                t = line.strip().split(",")
-                if len(t) >= 7 and t[1] == prec and t[2] == workload:
-                    return {"bytes": float(t[4]) + float(t[5]), "particles": float(t[3]), "kernel": t[0], "source": t[6]}
+        rows = {r[0]: r[1] for r in csv.reader(open(path)) if len(r) >= 2 and not r[0].startswith("#")}
+        f = lambda k: float(rows[k])
+        return {"kernel": rows["kernel"], "particles": f("particles_per_launch"),
+                "dram_bytes": f("dram__bytes_read.sum") + f("dram__bytes_write.sum"),
+                "flop_executed": f("flop_executed_per_launch"), "inst_per_particle": f("warp_inst_per_32_particles"),
+                "source": os.path.relpath(path, ROOT)}
     except Exception:
-        pass
-    return None
+        return None
 
 
-def _peaks():
+def _peaks_file():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             return json.load(f), "measured"
@@ -83,19 +94,17 @@ def _workload_desc(wl, shrink):
 
 
 # ------------------------------------------------------------------------------------------------
-# reference arm / cpu_baseline: the oracle on the host cores
+# reference arm / cpu_baseline: the oracle on the host cores (the only places bench.py touches oracle/)
 # ------------------------------------------------------------------------------------------------
-def _oracle_setup(name, shrink):
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from helpers import grid_from_domain, oracle_particles
+def _oracle_setup(wl):
     from oracle import oracle as O
+    from oracle.parity import grid_from_domain, oracle_particles
     O.build()
-    wl = _workload(name, shrink=shrink)
     rt = np.float32 if wl.dtype == "f32" else np.float64
     g = grid_from_domain(O, wl.dom)
     parts = [oracle_particles(O, sp, rt) for sp in wl.species]
     fields = {k: np.asarray(v, rt).astype(np.float64) for k, v in wl.fields.items()}
-    return O, wl, g, parts, fields
+    return O, g, parts, fields
 
 
 def _oracle_step(O, wl, g, parts, fields):
@@ -118,16 +127,19 @@ def _cpu_model():
     return "unknown"
 
 
-def cpu_baseline(name, shrink=16, steps=1):
-    O, wl, g, parts, fields = _oracle_setup(name, shrink)
+def cpu_baseline(name, wl_full=None):
+    """The oracle as it stands on ONE FULL step of the workload, all host cores; one single-thread figure on
+    a /8 sample; and the operation count of the method by code (oracle.count_ops on a small sample)."""
+    wl = wl_full if wl_full is not None else _workload(name)
+    O, g, parts, fields = _oracle_setup(wl)
     t0 = time.perf_counter()
-    n = 0
-    for _ in range(steps):
-        n += _oracle_step(O, wl, g, parts, fields)
+    n = _oracle_step(O, wl, g, parts, fields)
     dt = time.perf_counter() - t0
-    # one single-thread figure on a smaller sample
+    del parts
     nt = O.num_threads()
-    O1, wl1, g1, parts1, fields1 = _oracle_setup(name, shrink * 2)
+    wl1 = _workload(name, shrink=8)
+    O1, g1, parts1, fields1 = _oracle_setup(wl1)
+    cnt = O.count_ops(g1, parts1[0], fields1, wl1.dt)
     O.set_num_threads(1)
     t1 = time.perf_counter()
     n1 = _oracle_step(O1, wl1, g1, parts1, fields1)
@@ -135,8 +147,11 @@ def cpu_baseline(name, shrink=16, steps=1):
     O.set_num_threads(nt)
     return {"value": n / dt, "unit": UNIT, "cores": nt, "kind": "oracle", "cpu_model": _cpu_model(),
             "single_thread_value": n1 / dt1,
-            "sample": f"{steps} step(s) of {_workload_desc(wl, shrink)}; oracle = oracle/grpic_oracle.c "
-                      f"(FP64, OpenMP over particles), {dt:.1f} s"}
+            "ops_per_update_counted": cnt["total_per_update"],
+            "ops_per_update_by_stage": {k: round(v, 1) for k, v in cnt["per_stage"].items() if v > 0},
+            "sample": f"1 full step of {_workload_desc(wl, 1)}; oracle = oracle/grpic_oracle.c "
+                      f"(FP64, OpenMP over particles), {dt:.1f} s; single thread: 1 step of the /8 grid; operation count: "
+                      f"the same source on a counting type, {cnt['particles']} particles"}
 
 
 def run_reference(args):
@@ -144,7 +159,8 @@ def run_reference(args):
     if rank != 0:
         return
     shrink = 4
-    O, wl, g, parts, fields = _oracle_setup(args.workload, shrink)
+    wl = _workload(args.workload, shrink=shrink)
+    O, g, parts, fields = _oracle_setup(wl)
     for _ in range(args.warmup):
         _oracle_step(O, wl, g, parts, fields)
     t0 = time.perf_counter()
@@ -223,6 +239,159 @@ class ClockSampler:
         return out
 
 
+def measure_peaks(ctx, kinds=("ffma", "dfma", "mufu", "smem_rmw"), reps=5):
+    """Throughput of the register-only probes of the library (include/grpic.h grpic_probe), CUDA events around each
+    launch, best of `reps` after a warm-up: {"ffma": TFLOP/s, "dfma": TFLOP/s, "mufu": Tera thread-op/s, ...}."""
+    import torch
+    stream = torch.cuda.current_stream()
+    out = {}
+    for kind in kinds:
+        iters = {"ffma": 4096, "dfma": 2048, "mufu": 1024, "smem_rmw": 512}[kind]
+        best = None
+        for r in range(reps + 1):
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ops = ctx.probe(kind, iters, stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            if r > 0:
+                best = ms if best is None else min(best, ms)
+        out[kind] = ops / (best * 1e-3) / 1e12
+    return out
+
+
+def run_peaks(args):
+    import torch
+    from paper_2511_17701_b200 import grpic as G
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device"
+    sampler = ClockSampler(0)
+    ctx = G.Context(64, 64, 0.5, 1.5, 10.0, precision="f32")
+    time.sleep(0.5)
+    pk = measure_peaks(ctx, reps=8)
+    clocks = sampler.stop()
+    print(json.dumps({"peaks": {"fp32_fma_tflops": pk["ffma"], "fp64_fma_tflops": pk["dfma"],
+                                "mufu_rsqrt_tera_ops": pk["mufu"], "shared_rmw_tera_ops": pk["smem_rmw"]},
+                      "derived": {"fp32_fma_tflops": ALU_PEAK_DERIVED["f32"], "fp64_fma_tflops": ALU_PEAK_DERIVED["f64"],
+                                  "how": "148 SMs x 128 (FP32) / 64 (FP64) lanes x 2 x 1.965 GHz"},
+                      "how": "grpic_probe: 1184 x 256 threads, 8 independent chains per thread, CUDA events, best of 8",
+                      "clocks": clocks}))
+
+
+class DeviceRun:
+    """The resident workload and its step loop: what `value` times."""
+
+    def __init__(self, G, wl, prec, knobs=(), no_tile=False):
+        import torch
+        self.torch, self.G, self.wl, self.prec = torch, G, wl, prec
+        dom = wl.dom
+        names = ("D1", "D2", "D3", "B1", "B2", "B3")
+        self.ctx = ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
+        if no_tile:
+            ctx.set_int("tile_path", 0)
+        for kv in knobs:                       # ablation knobs of include/grpic.h, e.g. --set lanes_path=0
+            k, v = kv.split("=", 1)
+            (ctx.set_real if k in ("sort_lookahead", "small_angle") else ctx.set_int)(k, float(v) if "." in v else int(v))
+        self.fdev = G.grid_tensors(wl.fields, names, prec)
+        # the fused step keeps the previous position in registers: no *_prev columns; two column sets per species,
+        # swapped by the out-of-place sort (grpic_sort_into), so that a sort moves every byte once
+        self.sets = [G.ParticleSet.from_host(sp, prec).drop_prev() for sp in wl.species]
+        self.spare = [p.empty_like() for p in self.sets]
+        self.J = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
+        self.stream = torch.cuda.current_stream()
+        self.sort_every = wl.sort_every if wl.sort_every > 0 else 10
+        # the sort orders by the cell predicted half a sort interval ahead (include/grpic.h "sort_lookahead")
+        if not any(kv.startswith("sort_lookahead=") for kv in knobs):
+            ctx.set_real("sort_lookahead", 0.5 * self.sort_every)
+        self.it = 0
+
+    def one_step(self, evs=None, sevs=None):
+        torch = self.torch
+        launches = 0
+        if self.it % self.sort_every == 0:
+            for i in range(len(self.sets)):
+                if sevs is not None:
+                    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                    a.record(self.stream)
+                self.ctx.sort_into(self.sets[i], self.spare[i], self.stream)
+                self.sets[i], self.spare[i] = self.spare[i], self.sets[i]
+                launches += KERNELS_PER_SORT
+                if sevs is not None:
+                    b.record(self.stream); sevs.append((a, b))
+        for k in self.J.values():
+            k.zero_()
+        for p in self.sets:
+            if evs is not None:
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record(self.stream)
+            self.ctx.step(p, self.fdev, self.J, self.wl.dt, self.stream)
+            launches += KERNELS_PER_STEP_CALL
+            if evs is not None:
+                b.record(self.stream); evs.append((a, b))
+        self.it += 1
+        return launches
+
+    def timed(self, steps, warmup, barrier=lambda: None):
+        """W warm-up steps, then exactly K timed steps between synchronisations; device time by CUDA events."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.one_step()
+        torch.cuda.synchronize()
+        barrier()
+        upd0 = self.ctx.updates_total()
+        evs, sevs = [], []
+        t_a = torch.cuda.Event(enable_timing=True); t_b = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t_a.record(self.stream)
+        launches = 0
+        for _ in range(steps):
+            launches += self.one_step(evs, sevs)
+        t_b.record(self.stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms = t_a.elapsed_time(t_b)
+        updates = self.ctx.updates_total() - upd0
+        return dict(ms=ms, updates=updates, launches=launches,
+                    step_ms=sum(a.elapsed_time(b) for a, b in evs), n_step_calls=len(evs),
+                    sort_ms=sum(a.elapsed_time(b) for a, b in sevs), n_sorts=len(sevs))
+
+    def close(self):
+        self.ctx.close()
+        del self.sets, self.spare, self.J, self.fdev
+        self.torch.cuda.empty_cache()
+
+
+def roofline_of(prec, workload, r, peak_measured, peaks_file, peak_src, full_size, kernel):
+    """The `roofline` object of one timed run r (DeviceRun.timed)."""
+    upd_per_launch = r["updates"] / max(1, r["n_step_calls"])
+    sec_per_launch = r["step_ms"] * 1e-3 / max(1, r["n_step_calls"])
+    ach = FLOPS_PER_UPDATE_NITER10 * upd_per_launch / sec_per_launch / 1e12
+    hbm_ach = BYTES_PER_UPDATE[prec] * upd_per_launch / sec_per_launch / 1e9
+    prof = _profile_numbers(prec, workload) if full_size else None
+    out = {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak_measured, "unit": "TFLOP/s",
+           "frac": ach / peak_measured,
+           "frac_is": "ALGORITHMIC operations of the method at n_iter = 10 (2051 per update, DESIGN.md section 7; the two "
+                      "fixed-point loops leave early once an iterate repeats bit for bit, so fewer are executed) per second "
+                      "over the FMA peak measured in this run",
+           "peak_source": "measured in this run: grpic_probe FFMA/DFMA chains (CUDA events, best of 5)",
+           "peak_derived": ALU_PEAK_DERIVED[prec],
+           "flops_per_update": FLOPS_PER_UPDATE_NITER10, "updates_per_launch": upd_per_launch,
+           "ms_per_launch": sec_per_launch * 1e3, "kernel_share_of_step": r["step_ms"] / r["ms"],
+           "traffic": (prof["dram_bytes"] if prof else None),
+           "hbm": {"achieved": hbm_ach, "peak": peaks_file["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / peaks_file["hbm_gbs"],
+                   "bytes_per_update": BYTES_PER_UPDATE[prec], "peak_source": peak_src}}
+    if prof:
+        ex = prof["flop_executed"] / prof["particles"]
+        out["executed"] = {"flop_per_update": ex, "achieved": ex * upd_per_launch / sec_per_launch / 1e12,
+                           "frac": ex * upd_per_launch / sec_per_launch / 1e12 / peak_measured,
+                           "warp_inst_per_32_particles": prof["inst_per_particle"],
+                           "note": "FP instructions the kernel EXECUTES (2 x FFMA + FMUL + FADD of the committed ncu opcode "
+                                   "histogram) per second over the same measured peak"}
+        out["traffic_note"] = (f"dram__bytes_read.sum + dram__bytes_write.sum of one {prof['kernel']} launch over "
+                               f"{prof['particles']:.0f} particles, {prof['source']}")
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -235,92 +404,34 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
 
     wl = _workload(args.workload, seed_offset=rank, shrink=args.shrink)
     prec = wl.dtype if args.precision is None else args.precision
-    dom = wl.dom
-    names = ("D1", "D2", "D3", "B1", "B2", "B3")
-    ctx = G.Context(dom.n1, dom.n2, dom.a, dom.r_min, dom.r_max, nghost=dom.ng, precision=prec)
-    if args.no_tile:
-        ctx.set_int("tile_path", 0)
-    for kv in args.set:                        # ablation knobs of include/grpic.h, e.g. --set lanes_path=0
-        k, v = kv.split("=", 1)
-        (ctx.set_real if k in ("sort_lookahead", "small_angle") else ctx.set_int)(k, float(v) if "." in v else int(v))
-    fdev = G.grid_tensors(wl.fields, names, prec)
-    # the fused step keeps the previous position in registers: no *_prev columns; two column sets per species,
-    # swapped by the out-of-place sort (grpic_sort_into), so that a sort moves every byte once
-    sets = [G.ParticleSet.from_host(sp, prec).drop_prev() for sp in wl.species]
-    spare = [p.empty_like() for p in sets]
-    J = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec), device="cuda") for k in ("J1", "J2", "J3")}
-    stream = torch.cuda.current_stream()
-    sort_every = wl.sort_every if wl.sort_every > 0 else 10
-    # the sort orders by the cell predicted half a sort interval ahead (include/grpic.h "sort_lookahead"): the
-    # particles of a warp are then closest together in the middle of the interval, not right after the sort
-    ctx.set_real("sort_lookahead", 0.5 * sort_every)
-    n_total = sum(p.n for p in sets)
-
-    def one_step(it, evs=None):
-        launches = 0
-        if it % sort_every == 0:
-            for i in range(len(sets)):
-                ctx.sort_into(sets[i], spare[i], stream)
-                sets[i], spare[i] = spare[i], sets[i]
-                launches += 11
-        for k in J.values():
-            k.zero_()
-        for p in sets:
-            if evs is not None:
-                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-                a.record(stream)
-            ctx.step(p, fdev, J, wl.dt, stream)
-            launches += 1
-            if evs is not None:
-                b.record(stream)
-                evs.append((a, b))
-        return launches
-
-    it = 0
+    run = DeviceRun(G, wl, prec, knobs=args.set, no_tile=args.no_tile)
     sampler = ClockSampler(local) if rank == 0 else None      # nvidia-smi needs ~a second to start sampling
-    for _ in range(args.warmup):
-        one_step(it); it += 1
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    upd0 = ctx.updates_total()
-    evs = []
-    t_a = torch.cuda.Event(enable_timing=True); t_b = torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    t_a.record(stream)
-    launches = 0
-    for _ in range(args.steps):
-        launches += one_step(it, evs); it += 1
-    t_b.record(stream)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
+    r = run.timed(args.steps, args.warmup, barrier)
     clocks = sampler.stop() if sampler else None
-    ms = t_a.elapsed_time(t_b)
-    updates = ctx.updates_total() - upd0
-    step_kernel_ms = sum(a.elapsed_time(b) for a, b in evs)
-    counters = ctx.counters()
-
-    ms_max, updates_all = reduce_over_ranks(ms, updates, world)
+    counters = run.ctx.counters()
+    ms_max, updates_all = reduce_over_ranks(r["ms"], r["updates"], world)
+    # the ALU denominators, measured on this GPU right after the timed region
+    pk = measure_peaks(run.ctx, kinds=("ffma", "dfma")) if rank == 0 else None
 
     # ---- end to end through the host-buffer ABI call (pinned host memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
+        ctx = run.ctx
+        names = ("D1", "D2", "D3", "B1", "B2", "B3")
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
-        hwl = wl
-        hsets = [G.ParticleSet.from_host(sp, prec, device="cpu", pinned=True) for sp in hwl.species]
-        hf = G.grid_tensors(hwl.fields, names, prec, device="cpu", pinned=True)
+        hsets = [G.ParticleSet.from_host(sp, prec, device="cpu", pinned=True) for sp in wl.species]
+        hf = G.grid_tensors(wl.fields, names, prec, device="cpu", pinned=True)
         hJ = {k: torch.zeros(ctx.shape, dtype=G.torch_real(prec)).pin_memory() for k in ("J1", "J2", "J3")}
         up = down = 0
         for p in hsets:                      # warm-up: allocates the library's device chunks
             ctx.step_host(p, hf, hJ, wl.dt, with_prev=False)
         u0 = ctx.updates_total()
         torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
+        barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             for p in hsets:
@@ -334,53 +445,58 @@ def run_ours(args):
                "d2h_bytes_per_step": down // e2e_steps, "steps": e2e_steps,
                "api": "grpic_step_host (C ABI, pinned host buffers, chunked H2D -> fused step -> D2H on three streams; *_prev columns not requested)"}
         del hsets, hf, hJ
+    sort_every = run.sort_every
+    run.close()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    peaks, peak_src = _peaks()
-    value = updates_all / (ms_max * 1e-3)
-    n_step_launches = len(evs)
-    upd_per_launch = updates / max(1, n_step_launches)
-    sec_per_launch = step_kernel_ms * 1e-3 / max(1, n_step_launches)
-    flops = FLOPS_PER_UPDATE_NITER10 * upd_per_launch
-    ach_tflops = flops / sec_per_launch / 1e12
-    alu_peak = ALU_PEAK_TFLOPS[prec]
-    hbm_ach = BYTES_PER_UPDATE[prec] * upd_per_launch / sec_per_launch / 1e9
-    kernel = "k_step_tiled" if not args.no_tile else "k_push_or_step<.,true>"
-    tr = _ncu_traffic(prec, args.workload) if (not args.no_tile and args.shrink == 1) else None
+    peaks_file, peak_src = _peaks_file()
+    full = args.shrink == 1 and not args.no_tile and not args.set
+    kernel = "k_step_lanes (dense items) + k_step_tiled (sparse items)" if prec == "f32" and not args.no_tile else \
+             ("k_step_tiled" if not args.no_tile else "k_push_or_step<.,true>")
+    peak = pk["ffma"] if prec == "f32" else pk["dfma"]
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": prec, "data": "synthetic",
+        "metric": METRIC, "value": updates_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": _workload_desc(wl, args.shrink), "sort_every": sort_every,
                    "sort": "grpic_sort_into between two column sets per species; no *_prev columns (fused step); "
                            "sort_lookahead = sort_every/2",
                    "l2": "inputs (particle columns, several GB) larger than the 126 MB L2; no flush needed",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "paper_context": "paper: ~1.2-1.4e8 updates/s on 1x A100 (P:550), other hardware, not a target"},
-        "roofline": {"bound": "alu", "kernel": kernel, "achieved": ach_tflops, "peak": alu_peak, "unit": "TFLOP/s",
-                     "frac": ach_tflops / alu_peak, "traffic": (tr["bytes"] if tr else None),
-                     "traffic_note": (f"dram read+write bytes of one {tr['kernel']} launch over {tr['particles']:.0f} particles, "
-                                      f"{tr['source']}" if tr else None),
-                     "peak_source": f"derived: 148 SMs x {128 if prec == 'f32' else 64} lanes x 2 (FMA) x 1.965 GHz",
-                     "flops_per_update": FLOPS_PER_UPDATE_NITER10,
-                     "updates_per_launch": upd_per_launch, "ms_per_launch": sec_per_launch * 1e3,
-                     "kernel_share_of_step": step_kernel_ms / ms,
-                     "hbm": {"achieved": hbm_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                             "frac": hbm_ach / peaks["hbm_gbs"], "bytes_per_update": BYTES_PER_UPDATE[prec],
-                             "peak_source": peak_src}},
-        "without_sort": {"value": updates / (step_kernel_ms * 1e-3), "unit": UNIT,
-                         "note": "fused step launches only (CUDA events around each launch); `value` includes grpic_sort_into every sort_every steps and the J zero-fills"},
-        "clocks": clocks, "gpu_launches": launches,
+        "roofline": roofline_of(prec, args.workload, r, peak, peaks_file, peak_src, full, kernel),
+        "peaks_measured": {"fp32_fma_tflops": pk["ffma"], "fp64_fma_tflops": pk["dfma"]},
+        "without_sort": {"value": r["updates"] / (r["step_ms"] * 1e-3), "unit": UNIT,
+                         "note": "fused step calls only (CUDA events around each grpic_step); `value` includes grpic_sort_into every sort_every steps and the J zero-fills"},
+        "sort": {"ms_per_call": r["sort_ms"] / max(1, r["n_sorts"]), "calls": r["n_sorts"],
+                 "note": "grpic_sort_into of one species (CUDA events around the call; no host synchronisation inside)"},
+        "clocks": clocks, "gpu_launches": r["launches"],
         "counters_last_step": counters, "updates_timed": updates_all,
     }
     if e2e is not None:
         out["e2e"] = e2e
+    # the other single-GPU configurations of BASELINE.json, each as a short run of the same loop (config 5 in FP64)
+    if world == 1 and not args.no_others and args.workload == "large" and full:
+        others = []
+        for name in ("magnetosphere", "two_species"):
+            w2 = _workload(name)
+            run2 = DeviceRun(G, w2, w2.dtype)
+            r2 = run2.timed(min(args.steps, 20), 3)
+            rf = roofline_of(w2.dtype, name, r2, pk["ffma"] if w2.dtype == "f32" else pk["dfma"], peaks_file, peak_src, True,
+                             "k_step_lanes + k_step_tiled" if w2.dtype == "f32" else "k_step_tiled")
+            others.append({"workload": _workload_desc(w2, 1), "dtype": w2.dtype, "steps": min(args.steps, 20),
+                           "value": r2["updates"] / (r2["ms"] * 1e-3), "unit": UNIT, "ms_per_step": r2["ms"] / min(args.steps, 20),
+                           "ms_per_launch": rf["ms_per_launch"], "frac": rf["frac"], "peak": rf["peak"],
+                           "hbm_frac": rf["hbm"]["frac"], "executed": rf.get("executed")})
+            run2.close()
+            del w2
+        out["other_workloads"] = others
     if world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.workload, shrink=4, steps=16)
+        out["cpu_baseline"] = cpu_baseline(args.workload, wl_full=wl if args.shrink == 1 else None)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -398,11 +514,15 @@ def main():
     ap.add_argument("--no-tile", action="store_true", help="force the direct kernel")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of configs 3 and 5")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--peaks", action="store_true", help="print the measured FFMA / DFMA / MUFU / shared-RMW peaks and exit")
     ap.add_argument("--set", action="append", default=[], metavar="KEY=VALUE",
                     help="grpic_set_int / grpic_set_real knob for ablation runs (repeatable)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.peaks:
+        run_peaks(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

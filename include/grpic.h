@@ -184,6 +184,15 @@ int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_absorbed_in, int
  * the numerator of the throughput metric.  Synchronises `cuda_stream`. */
 int grpic_updates_total(grpic_ctx* ctx, int64_t* n_updates, void* cuda_stream);
 
+/* Throughput probes: the measured denominators of the ALU roofline (bench.py --peaks and every bench line).  Enqueues ONE
+ * launch of a register-only kernel on `cuda_stream` (1184 blocks x 256 threads, 8 independent chains per thread) and
+ * returns in *ops the operations that launch executes; the caller times it with CUDA events.
+ *   "ffma": FP32 fused multiply-adds, *ops in flop (2 per FMA);  "dfma": FP64 likewise;
+ *   "mufu": rsqrt.approx.f32 (special-function unit), *ops in thread operations;
+ *   "smem_rmw": LDS + FADD + STS on lane-private shared words (the read-modify-write of k_step_lanes' windows).
+ * Errors: EINVAL, ECUDA. */
+int grpic_probe(grpic_ctx* ctx, const char* what, int64_t iters, int64_t* ops, void* cuda_stream);
+
 /* ---- Field-solver half of the step (Sec. 3.3).  Grid kernels; same array layout; device pointers. ----
  * The caller sequences them and the time levels (Sec. 3.4) and fills the ghost ROWS i < 0, i >= n1 of the inputs
  * (P:461-467); ghost columns beyond the axes are not read.  Rows written: every row whose x1-stencil lies inside the

@@ -13,7 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
-_SOURCES = ["grpic.cu", "grpic_kernels.cuh", "grpic_device.cuh", "grpic_tiled.cuh", "grpic_lanes.cuh", "grpic_fields.cuh"]
+_SOURCES = ["grpic.cu", "grpic_kernels.cuh", "grpic_device.cuh", "grpic_tiled.cuh", "grpic_lanes.cuh", "grpic_fields.cuh", "grpic_probe.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC", "--cudart", "static"]

@@ -18,6 +18,7 @@
 #include "grpic_tiled.cuh"
 #include "grpic_lanes.cuh"
 #include "grpic_fields.cuh"
+#include "grpic_probe.cuh"
 
 using namespace grpic;
 typedef grpic_real real;
@@ -731,6 +732,23 @@ int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_in, int64_t* n_o
   if (n_in) *n_in = (int64_t)h[1];
   if (n_out) *n_out = (int64_t)h[2];
   if (n_over) *n_over = (int64_t)h[3];
+  return GRPIC_OK;
+}
+
+int grpic_probe(grpic_ctx* ctx, const char* what, int64_t iters, int64_t* ops, void* stream) {
+  if (!ctx || !what || !ops) return fail(ctx, GRPIC_EINVAL, "NULL argument");
+  if (int rd = check_device(ctx)) return rd;
+  if (iters < 1 || iters > (1 << 24)) return fail(ctx, GRPIC_EINVAL, "iters must be in 1..2^24");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int grid = 148 * 8;
+  float* out = reinterpret_cast<float*>(ctx->d_counters + 6);            // a spare word, never written in practice
+  const int64_t lane_ops = (int64_t)grid * kProbeBlock * kProbeChains * 8 * iters;
+  if (!std::strcmp(what, "ffma")) { k_probe<0><<<grid, kProbeBlock, 0, st>>>((int)iters, 1.0f, out); *ops = 2 * lane_ops; }
+  else if (!std::strcmp(what, "dfma")) { k_probe<1><<<grid, kProbeBlock, 0, st>>>((int)iters, 1.0f, out); *ops = 2 * lane_ops; }
+  else if (!std::strcmp(what, "mufu")) { k_probe<2><<<grid, kProbeBlock, 0, st>>>((int)iters, 1.0f, out); *ops = lane_ops; }
+  else if (!std::strcmp(what, "smem_rmw")) { k_probe<3><<<grid, kProbeBlock, 0, st>>>((int)iters, 1.0f, out); *ops = lane_ops; }
+  else return fail(ctx, GRPIC_EINVAL, std::string("unknown probe: ") + what);
+  CK(cudaGetLastError());
   return GRPIC_OK;
 }
 

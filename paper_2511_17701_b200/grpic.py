@@ -23,7 +23,8 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_interp_push", "grpic_deposit", "grpic_step", "grpic_sort", "grpic_tile_size",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
-           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into", "grpic_field_match"]
+           "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into", "grpic_field_match",
+           "grpic_probe"]
 
 
 class GrpicError(RuntimeError):
@@ -90,6 +91,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_sort_into.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Particles), _vp]
     lib.grpic_counters.argtypes = [_vp] + [C.POINTER(C.c_int64)] * 4 + [_vp]
     lib.grpic_updates_total.argtypes = [_vp, C.POINTER(C.c_int64), _vp]
+    lib.grpic_probe.argtypes = [_vp, C.c_char_p, C.c_int64, C.POINTER(C.c_int64), _vp]
     lib.grpic_step_host.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(_Fields), C.POINTER(_Current), C.c_double,
                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.grpic_aux_fields.argtypes = [_vp, C.POINTER(_Fields), C.POINTER(_Vec3), C.POINTER(_Vec3), _vp]
@@ -307,6 +309,12 @@ class Context:
         v = [C.c_int64(0) for _ in range(4)]
         self._ck(self.lib.grpic_counters(self.h, *[C.byref(x) for x in v], _stream_ptr(stream)))
         return dict(zip(("alive", "absorbed_in", "absorbed_out", "overstep"), (int(x.value) for x in v)))
+
+    def probe(self, what: str, iters: int, stream=None) -> int:
+        """enqueue one throughput-probe launch ("ffma", "dfma", "mufu", "smem_rmw"); returns its operation count"""
+        v = C.c_int64(0)
+        self._ck(self.lib.grpic_probe(self.h, what.encode(), int(iters), C.byref(v), _stream_ptr(stream)))
+        return int(v.value)
 
     def updates_total(self, stream=None) -> int:
         v = C.c_int64(0)

@@ -29,7 +29,7 @@ def W():
 def pytest_terminal_summary(terminalreporter):
     """Evidence for the two FP32 allowances of the parity rules, printed with every GPU run."""
     try:
-        import helpers
+        from oracle import parity as helpers
         rows = helpers.AXIS_STATS
     except Exception:
         return
