@@ -830,6 +830,65 @@ def test_gauss_law_is_kept_by_the_closed_loop_on_the_gpu(G, O, W):
     print("Gauss-law drift after 30 steps:", drift, "scale", scale, "absorbed", absorbed)
 
 
+@pytest.mark.parametrize("prec,dense_min,look", [("f32", 2048, 0.0), ("f32", 4, 3.0), ("f64", 4, 3.0), ("f64", 1024, 0.0)])
+def test_lanes_kernel_dense_and_degenerate_items(G, O, W, prec, dense_min, look):
+    """k_step_lanes (one particle run per lane, lane-private J windows, 128-bit column blocks) against the oracle, in
+    both precisions (FP64 switched on explicitly): dense_min = 4 sends EVERY work item through it - items of a handful
+    of particles, runs of one partial block, items that begin and end inside a 16-byte block - and six steps without a
+    re-sort let the particles drift out of the windows (the strays take the L2 path).  Species without *_prev columns,
+    two column sets, look-ahead sort as in bench.py; then a species truncated to its alive count after the sort."""
+    wl = W.config_large(shrink=16)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, prec)
+    ctx.set_int("lanes_path", 1)
+    ctx.set_int("dense_min", dense_min)
+    fdev, fhost = _fields_both(G, wl, prec)
+    for sp in wl.species:
+        rng = np.random.default_rng(3)
+        sp.tag = sp.tag.copy(); sp.tag[rng.random(sp.n) < 0.03] = 0          # dead slots: ragged item boundaries
+        src = G.ParticleSet.from_host(sp, prec).drop_prev()
+        ps = src.empty_like()
+        ctx.sort_into(src, ps)
+        ctx.set_real("sort_lookahead", look)
+        for step in range(6):
+            if step == 2:
+                ctx.sort_into(ps, src)                # now with a dt: the look-ahead key
+                ps, src = src, ps
+            res, c = _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, prec, "fused")
+        print("lanes", prec, dense_min, look, res, c)
+        # compaction: drop the dead tail (p->n < n at the sort): the table still covers [0, n_alive)
+        ctx.sort_into(ps, src)
+        n_alive = ctx.sorted_alive(src)
+        cut = G.ParticleSet({k: (None if v is None else v[:n_alive]) for k, v in src.cols.items()},
+                            src.q_over_m, src.charge, src.massive)
+        res, c = _one_step_parity(G, O, ctx, g, cut, fdev, fhost, wl.dt, prec, "fused")
+        assert c["alive"] + c["absorbed_in"] + c["absorbed_out"] == n_alive
+
+
+def test_lanes_kernel_declines_unaligned_columns(G, O, W):
+    """Columns that are only 4-byte aligned (views one element into a buffer): grpic_step must not take the 128-bit
+    block path (include/grpic.h asks for 16-byte alignment; the library checks instead of trusting) and still be right."""
+    import torch
+    wl = W.config_magnetosphere(shrink=16)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, "f32")
+    fdev, fhost = _fields_both(G, wl, "f32")
+    base = G.ParticleSet.from_host(wl.species[0], "f32").drop_prev()
+    cols = {}
+    for k, v in base.cols.items():
+        if v is None:
+            cols[k] = None
+            continue
+        buf = torch.empty(v.numel() + 8, dtype=v.dtype, device="cuda")
+        buf[1:1 + v.numel()] = v
+        cols[k] = buf[1:1 + v.numel()]
+    ps = G.ParticleSet(cols, base.q_over_m, base.charge, base.massive)
+    assert ps.cols["dx1"].data_ptr() % 16 != 0
+    ctx.sort(ps)
+    for step in range(2):
+        _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, "f32", "fused")
+
+
 @pytest.mark.parametrize("prec", ["f32", "f64"])
 def test_injection_and_compaction_after_a_sort(G, O, W, prec):
     """after grpic_sort the alive particles sit in [0, n_alive) (grpic_sorted_alive).  Particles written
