@@ -292,7 +292,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->k_J = 4.0 * M_PI;                                    // coefficient of J in Ampere's law (Eq. 37)
   ctx->n_iter = 10;
   ctx->tile_path = 1;
-  ctx->lanes_path = sizeof(real) == 4 ? 1 : 0;             // FP64: measured slower than k_step_tiled (1 CTA of 256 per SM)
+  ctx->lanes_path = 1;
   ctx->dense_min = 2048;
   ctx->lanes_attr[0] = ctx->lanes_attr[1] = false;
   ctx->tiled_attr[0][0] = ctx->tiled_attr[0][1] = ctx->tiled_attr[1][0] = ctx->tiled_attr[1][1] = false;

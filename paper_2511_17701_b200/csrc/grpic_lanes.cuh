@@ -24,10 +24,18 @@
 
 namespace grpic {
 
-#ifndef GRPIC_LANES_BLOCK
-#define GRPIC_LANES_BLOCK 256
+// Lanes (= particle runs) per work item and particles per 16-byte block of a real column, by precision.  FP32: 256 lanes,
+// two items resident per SM (128 registers); blocks of four.  FP64: 384 lanes, one item per SM (12 warps instead of the
+// 8 of k_step_tiled<double>: the FP64 step is bound by dependent-issue latency, so resident warps are what it needs);
+// blocks of two, so that a lane's staging slot and window (512 bytes) leave room for them in the 227 KB of the SM.
+#ifndef GRPIC_LANES_BLOCK32
+#define GRPIC_LANES_BLOCK32 256
 #endif
-constexpr int kLThreads = GRPIC_LANES_BLOCK;   // lanes (= particle runs) per work item
+#ifndef GRPIC_LANES_BLOCK64
+#define GRPIC_LANES_BLOCK64 384
+#endif
+template <typename T> constexpr int kLThreads = sizeof(T) == 4 ? GRPIC_LANES_BLOCK32 : GRPIC_LANES_BLOCK64;
+template <typename T> constexpr int kLPB = 16 / (int)sizeof(T);      // particles per block
 constexpr int kLWin = 3;                       // cells per edge of a lane's private J window
 constexpr int kLVals = 3 * 16;                 // slots of a window: [component][4][4] nodes
 #ifndef GRPIC_LANES_QUAD
@@ -38,19 +46,21 @@ constexpr int kLQuad = GRPIC_LANES_QUAD;       // lanes that interleave their 16
 #define GRPIC_LANES_PREFETCH 1
 #endif
 constexpr bool kLPrefetch = GRPIC_LANES_PREFETCH != 0;
-static_assert(kLVals * kLThreads >= kRawElems, "the raw field stencil is staged in the space of the lane windows");
+static_assert(kLVals * kLThreads<float> >= kRawElems && kLVals * kLThreads<double> >= kRawElems,
+              "the raw field stencil is staged in the space of the lane windows");
 
 template <typename T>
 constexpr size_t lanes_smem_bytes() {
-  return (size_t)(kLVals * kLThreads + kNodeElems + 7 * 4 * kLThreads) * sizeof(T) + (size_t)(2 * 4 + 1) * kLThreads * 4 + 16 +
+  // windows + node tile + staged real columns (7 x 16 bytes per lane) + staged cell indices + barrier + sort-key offsets
+  return (size_t)(kLVals * kLThreads<T> + kNodeElems<T>) * sizeof(T) + (size_t)kLThreads<T> * (7 * 16 + 2 * 4 * kLPB<T>) + 16 +
          (size_t)(kTile * kTile + 4) * 4;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -61,7 +71,7 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 // Eight plain read-modify-writes of one deposit segment (layout of deposit_segments) of cell (c1, c2):
 template <typename T>
 __device__ __forceinline__ void lane_add8(T* pW, int c1, int c2, const T v[8]) {
-  constexpr int S = kLThreads;
+  constexpr int S = kLThreads<T>;
   const int r0 = (c1 & 3) * 4, r1 = ((c1 + 1) & 3) * 4, q0 = c2 & 3, q1 = (c2 + 1) & 3;
   T* const p00 = pW + (r0 + q0) * S;
   T* const p01 = pW + (r0 + q1) * S;
@@ -79,14 +89,14 @@ struct LaneCell {
   T *p00, *p01, *p10, *p11;
   T o[8];
   __device__ __forceinline__ void load(T* pW, int c1, int c2) {
-    constexpr int S = kLThreads;
+    constexpr int S = kLThreads<T>;
     const int r0 = (c1 & 3) * 4, r1 = ((c1 + 1) & 3) * 4, q0 = c2 & 3, q1 = (c2 + 1) & 3;
     p00 = pW + (r0 + q0) * S; p01 = pW + (r0 + q1) * S; p10 = pW + (r1 + q0) * S; p11 = pW + (r1 + q1) * S;
     o[0] = p00[0]; o[1] = p01[0]; o[2] = p00[16 * S]; o[3] = p10[16 * S];
     o[4] = p00[32 * S]; o[5] = p10[32 * S]; o[6] = p01[32 * S]; o[7] = p11[32 * S];
   }
   __device__ __forceinline__ void add_store(const T v[8]) const {
-    constexpr int S = kLThreads;
+    constexpr int S = kLThreads<T>;
     p00[0] = o[0] + v[0]; p01[0] = o[1] + v[1]; p00[16 * S] = o[2] + v[2]; p10[16 * S] = o[3] + v[3];
     p00[32 * S] = o[4] + v[4]; p10[32 * S] = o[5] + v[5]; p01[32 * S] = o[6] + v[6]; p11[32 * S] = o[7] + v[7];
   }
@@ -96,12 +106,13 @@ struct LaneCell {
 // No bounds test: a slot whose node lies outside the arrays is never written (no cell there), so it stays zero.
 template <typename T>
 __device__ __forceinline__ void lane_flush_node(const Consts<T>& g, const JPtrs<T>& J, T* pW, int n1, int n2) {
-  T* const w = pW + (((n1 & 3) * 4) + (n2 & 3)) * kLThreads;
+  constexpr int S = kLThreads<T>;
+  T* const w = pW + (((n1 & 3) * 4) + (n2 & 3)) * S;
   const int64_t a = (int64_t)(n1 + g.ng) * g.ld + (n2 + g.ng);
-  const T v0 = w[0], v1 = w[16 * kLThreads], v2 = w[32 * kLThreads];
+  const T v0 = w[0], v1 = w[16 * S], v2 = w[32 * S];
   if (v0 != T(0)) { red_add(J.j[0] + a, v0); w[0] = T(0); }
-  if (v1 != T(0)) { red_add(J.j[1] + a, v1); w[16 * kLThreads] = T(0); }
-  if (v2 != T(0)) { red_add(J.j[2] + a, v2); w[32 * kLThreads] = T(0); }
+  if (v1 != T(0)) { red_add(J.j[1] + a, v1); w[16 * S] = T(0); }
+  if (v2 != T(0)) { red_add(J.j[2] + a, v2); w[32 * S] = T(0); }
 }
 // the whole window with origin cell (wo1, wo2)
 template <typename T>
@@ -120,19 +131,19 @@ __device__ __forceinline__ void lane_flush_col(const Consts<T>& g, const JPtrs<T
 }
 
 template <typename T, typename CoordT = Coord<T>>
-__global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
+__global__ void __launch_bounds__(kLThreads<T>, (sizeof(T) == 4 ? 2 : 1))
     k_step_lanes(const Consts<T> g, const PPtrs<T> P, const FPtrs<T> F, const JPtrs<T> J, const SpeciesConst sc,
                  unsigned long long* counters, const WorkItem* items, const uint32_t* dense_idx,
                  const uint32_t* n_dense_ptr, const uint32_t* offsets, int nt2, int use_tma,
                  const __grid_constant__ FieldMaps maps) {
-  constexpr int NT = kLThreads;
+  constexpr int NT = kLThreads<T>;
+  constexpr int PB = kLPB<T>;                          // particles per block: 4 (FP32) or 2 (FP64)
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sW = reinterpret_cast<T*>(smem_raw_);            // raw stencil first, then the lane windows [slot][thread]
   T* sN = sW + kLVals * NT;                           // node-major averaged fields
-  T* sR = sN + kNodeElems;                            // staged real columns [7][thread][4]: dx1 dx2 u1 u2 u3 phi w
-  int32_t* sI = reinterpret_cast<int32_t*>(sR + 7 * 4 * NT);   // staged cell indices [2][thread][4]
-  uint32_t* sT = reinterpret_cast<uint32_t*>(sI + 2 * 4 * NT); // staged tags: four bytes per thread
-  uint64_t* bar = reinterpret_cast<uint64_t*>(sT + NT);
+  T* sR = sN + kNodeElems<T>;                            // staged real columns [7][thread][PB]: dx1 dx2 u1 u2 u3 phi w
+  int32_t* sI = reinterpret_cast<int32_t*>(sR + 7 * PB * NT);  // staged cell indices [2][thread][PB]
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sI + 2 * PB * NT);
   uint32_t* sO = reinterpret_cast<uint32_t*>(bar + 2);         // first slot of each of the tile's 256 sort keys, + end
 
   if (blockIdx.x >= n_dense_ptr[0]) return;
@@ -170,10 +181,10 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   for (int n = tid; n < kNodeW * kNodeW; n += NT) {
     const int w1 = n / kNodeW, w2 = n % kNodeW;
     const RawAcc<T> acc{sW, w1 + 1, w2 + 1 + off2};
-    T* o = sN + n * kNodeStride;
+    T* o = sN + n * kNodeStride<T>;
 #pragma unroll
     for (int c = 0; c < 6; ++c) o[c] = node_value<T>(acc, c, yee_kind(c), 0, 0);
-    o[6] = T(0); o[7] = T(0);
+    if (kNodeStride<T> == 8) { o[6] = T(0); o[7] = T(0); }
   }
   __syncthreads();
   T* const pW = sW + tid;                              // this lane's window: slot s at pW[s * NT]
@@ -186,7 +197,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   const T inv_dt = T(1) / dt;
   const T chg = (T)sc.charge;
   const uint32_t begin = item.begin, end = item.begin + item.count;
-  const uint32_t B0 = begin >> 2, B1 = (end + 3u) >> 2;
+  const uint32_t B0 = begin / PB, B1 = (end + PB - 1u) / PB;
   const uint32_t bpl = (B1 - B0 + NT - 1) / NT;        // blocks per lane
   // kLQuad consecutive lanes share a contiguous region of kLQuad * bpl blocks and take its blocks in turn: one warp
   // instruction then reads (writes) kLQuad * 16 contiguous bytes per group - whole 32-byte sectors and whole
@@ -194,9 +205,9 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   const uint32_t b_first = B0 + (uint32_t)(tid / kLQuad) * (bpl * kLQuad) + (uint32_t)(tid % kLQuad);
   // processing order of the four staged particles: slot = j ^ swz makes the scalar staging reads of a warp
   // hit 32 different banks
-  const int swz = (tid >> (sizeof(T) == 4 ? 3 : 2)) & 3;
-  T* const myR = sR + tid * 4;                         // column c at myR[c * 4 * NT + slot]
-  int32_t* const myI = sI + tid * 4;
+  const int swz = (tid >> 3) & (PB - 1);
+  T* const myR = sR + tid * PB;                        // column c at myR[c * PB * NT + slot]
+  int32_t* const myI = sI + tid * PB;
   unsigned n_alive = 0, n_in = 0, n_out = 0, n_over = 0;
   // The window follows the SORTED cell of the run: the particles of one sort key are contiguous, and
   // offsets[key] (the scanned histogram of the sort, kept per species) is where each key starts, so the lane knows
@@ -207,7 +218,7 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   const uint32_t* const offs = sO;                     // keys of this tile: offs[0 .. 256]
   uint32_t key = 0, next_b = 0;
   if (b_first < B1) {                                  // key of the run's first particle: offs[key] <= k < offs[key + 1]
-    const uint32_t kf = max(b_first << 2, begin);
+    const uint32_t kf = max(b_first * PB, begin);
     uint32_t lo = 0, hi = kTile * kTile;
 #pragma unroll 1
     while (hi - lo > 1u) {
@@ -222,8 +233,8 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
   T* const wcol[6] = {P.dx1, P.dx2, P.u1, P.u2, P.u3, P.phi};
 
   for (uint32_t b = b_first, bi = 0; bi < bpl && b < B1; ++bi, b += kLQuad) {
-    const uint32_t k0 = b << 2;
-    const bool full = k0 >= begin && k0 + 4u <= end;
+    const uint32_t k0 = b * PB;
+    const bool full = k0 >= begin && k0 + PB <= end;
     {                                                  // move the window to the sorted cell of this block
       const uint32_t kb = max(k0, begin);
       while (kb >= next_b) { ++key; next_b = offs[key + 1]; }
@@ -236,20 +247,16 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
       wo1 = n1; wo2 = n2;
     }
     // ---- stage in ----
+    uint32_t tags;                                     // one byte per particle of the block
     if (full) {
-      cp_async16(myI, P.i1 + k0);
-      cp_async16(myI + 4 * NT, P.i2 + k0);
+      if (PB == 4) { cp_async16(myI, P.i1 + k0); cp_async16(myI + PB * NT, P.i2 + k0); }
+      else { cp_async8(myI, P.i1 + k0); cp_async8(myI + PB * NT, P.i2 + k0); }
 #pragma unroll
-      for (int c = 0; c < 7; ++c) {
-        if (c == 5 && !sc.has_phi) continue;
-        const char* src = reinterpret_cast<const char*>(rcol[c] + k0);
-        char* dst = reinterpret_cast<char*>(myR + c * 4 * NT);
-#pragma unroll
-        for (int q = 0; q < (int)sizeof(T) / 4; ++q) cp_async16(dst + 16 * q, src + 16 * q);
-      }
-      cp_async4(sT + tid, P.tag + k0);
+      for (int c = 0; c < 7; ++c)
+        if (c != 5 || sc.has_phi) cp_async16(myR + c * PB * NT, rcol[c] + k0);
+      tags = PB == 4 ? *reinterpret_cast<const uint32_t*>(P.tag + k0) : (uint32_t)*reinterpret_cast<const uint16_t*>(P.tag + k0);
       if (kLPrefetch && (tid & 1) == 0 && bi + 1 < bpl && b + kLQuad < B1) {   // this lane's next block: in L2 by then
-        constexpr uint32_t nx = 4 * kLQuad;
+        constexpr uint32_t nx = PB * kLQuad;
         prefetch_l2(P.i1 + k0 + nx); prefetch_l2(P.i2 + k0 + nx);
 #pragma unroll
         for (int c = 0; c < 7; ++c)
@@ -257,31 +264,29 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
       }
       cp_async_wait_all();
     } else {
-      uint32_t tg = 0;
+      tags = 0;
 #pragma unroll
-      for (int s = 0; s < 4; ++s) {
+      for (int s = 0; s < PB; ++s) {
         const uint32_t k = k0 + s;
         if (k >= begin && k < end) {
-          myI[s] = P.i1[k]; myI[4 * NT + s] = P.i2[k];
+          myI[s] = P.i1[k]; myI[PB * NT + s] = P.i2[k];
 #pragma unroll
           for (int c = 0; c < 7; ++c)
-            if (c != 5 || sc.has_phi) myR[c * 4 * NT + s] = rcol[c][k];
-          tg |= (uint32_t)P.tag[k] << (8 * s);
+            if (c != 5 || sc.has_phi) myR[c * PB * NT + s] = rcol[c][k];
+          tags |= (uint32_t)P.tag[k] << (8 * s);
         }
       }
-      sT[tid] = tg;
     }
-    uint32_t tags = sT[tid];
-    // ---- the four particles ----
+    // ---- the particles of the block ----
 #pragma unroll 1
-    for (int j = 0; j < 4; ++j) {
+    for (int j = 0; j < PB; ++j) {
       const int s = j ^ swz;
       if (((tags >> (8 * s)) & 0xffu) == 0u) continue;  // dead, or not of this item
       const uint32_t k = k0 + s;
       PState<T> p;
-      p.i1 = myI[s]; p.i2 = myI[4 * NT + s];
-      p.dx1 = myR[s]; p.dx2 = myR[4 * NT + s];
-      p.u1 = myR[2 * 4 * NT + s]; p.u2 = myR[3 * 4 * NT + s]; p.u3 = myR[4 * 4 * NT + s];
+      p.i1 = myI[s]; p.i2 = myI[PB * NT + s];
+      p.dx1 = myR[s]; p.dx2 = myR[PB * NT + s];
+      p.u1 = myR[2 * PB * NT + s]; p.u2 = myR[3 * PB * NT + s]; p.u3 = myR[4 * PB * NT + s];
       const int ia = p.i1, ja = p.i2;
       const T xa = p.dx1, ya = p.dx2;
       if (P.i1p) { P.i1p[k] = ia; P.i2p[k] = ja; P.dx1p[k] = xa; P.dx2p[k] = ya; }
@@ -306,17 +311,17 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
       const bool a_win = dep && (unsigned)(ia - wo1) < (unsigned)kLWin && (unsigned)(ja - wo2) < (unsigned)kLWin;
       LaneCell<T> wa;
       if (a_win) wa.load(pW, ia, ja);
-      myI[s] = p.i1; myI[4 * NT + s] = p.i2;
-      myR[s] = p.dx1; myR[4 * NT + s] = p.dx2;
-      myR[2 * 4 * NT + s] = p.u1; myR[3 * 4 * NT + s] = p.u2; myR[4 * 4 * NT + s] = p.u3;
-      if (sc.has_phi) myR[5 * 4 * NT + s] += dt * dphidt;
+      myI[s] = p.i1; myI[PB * NT + s] = p.i2;
+      myR[s] = p.dx1; myR[PB * NT + s] = p.dx2;
+      myR[2 * PB * NT + s] = p.u1; myR[3 * PB * NT + s] = p.u2; myR[4 * PB * NT + s] = p.u3;
+      if (sc.has_phi) myR[5 * PB * NT + s] += dt * dphidt;
       if (res != 0) { tags &= ~(0xffu << (8 * s)); continue; }
       if (over) { ++n_over; continue; }
       T v3 = dphidt;
       if (reflected)
         v3 = v3_at_path_midpoint<T, CoordT>(g, ia, ja, T(0.5) * (xa + (T)di + p.dx1), T(0.5) * (ya + (T)dj + p.dx2),
                                             p.u1, p.u2, p.u3, eps);
-      const T qw = chg * myR[6 * 4 * NT + s];
+      const T qw = chg * myR[6 * PB * NT + s];
       T seg[2][8];
       deposit_segments(di, dj, xa, ya, p.dx1, p.dx2, qw * inv_dt, qw, v3, seg);
       const bool cross = (di != 0) || (dj != 0);
@@ -339,26 +344,28 @@ __global__ void __launch_bounds__(kLThreads, (sizeof(T) == 4 ? 2 : 1))
     }
     // ---- stage out ----
     if (full) {
-      *reinterpret_cast<uint4*>(P.i1 + k0) = *reinterpret_cast<const uint4*>(myI);
-      *reinterpret_cast<uint4*>(P.i2 + k0) = *reinterpret_cast<const uint4*>(myI + 4 * NT);
-#pragma unroll
-      for (int c = 0; c < 6; ++c) {
-        if (c == 5 && !sc.has_phi) continue;
-        const uint4* src = reinterpret_cast<const uint4*>(myR + c * 4 * NT);
-        uint4* dst = reinterpret_cast<uint4*>(wcol[c] + k0);
-#pragma unroll
-        for (int q = 0; q < (int)sizeof(T) / 4; ++q) dst[q] = src[q];
+      if (PB == 4) {
+        *reinterpret_cast<uint4*>(P.i1 + k0) = *reinterpret_cast<const uint4*>(myI);
+        *reinterpret_cast<uint4*>(P.i2 + k0) = *reinterpret_cast<const uint4*>(myI + PB * NT);
+        *reinterpret_cast<uint32_t*>(P.tag + k0) = tags;
+      } else {
+        *reinterpret_cast<uint2*>(P.i1 + k0) = *reinterpret_cast<const uint2*>(myI);
+        *reinterpret_cast<uint2*>(P.i2 + k0) = *reinterpret_cast<const uint2*>(myI + PB * NT);
+        *reinterpret_cast<uint16_t*>(P.tag + k0) = (uint16_t)tags;
       }
-      *reinterpret_cast<uint32_t*>(P.tag + k0) = tags;
+#pragma unroll
+      for (int c = 0; c < 6; ++c)
+        if (c != 5 || sc.has_phi)
+          *reinterpret_cast<uint4*>(wcol[c] + k0) = *reinterpret_cast<const uint4*>(myR + c * PB * NT);
     } else {
 #pragma unroll
-      for (int s = 0; s < 4; ++s) {
+      for (int s = 0; s < PB; ++s) {
         const uint32_t k = k0 + s;
         if (k >= begin && k < end) {
-          P.i1[k] = myI[s]; P.i2[k] = myI[4 * NT + s];
+          P.i1[k] = myI[s]; P.i2[k] = myI[PB * NT + s];
 #pragma unroll
           for (int c = 0; c < 6; ++c)
-            if (c != 5 || sc.has_phi) wcol[c][k] = myR[c * 4 * NT + s];
+            if (c != 5 || sc.has_phi) wcol[c][k] = myR[c * PB * NT + s];
           P.tag[k] = (uint8_t)((tags >> (8 * s)) & 0xffu);
         }
       }
@@ -404,7 +411,7 @@ bool launch_step_lanes(const TmaEncoder& enc, bool want_tma, const Consts<T>& g,
   for (int c = 0; c < 6 && use_tma; ++c)
     if (!enc.encode(&maps.m[c], F.f[c], (int)sizeof(T), rows, g.ld)) use_tma = 0;
   const int nt2 = (g.n2 + kTile - 1) / kTile;
-  k_step_lanes<T, CoordT><<<max_dense, kLThreads, lanes_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, dense_idx,
+  k_step_lanes<T, CoordT><<<max_dense, kLThreads<T>, lanes_smem_bytes<T>(), st>>>(g, P, F, J, sc, counters, items, dense_idx,
                                                                               d_n_dense, offsets, nt2, use_tma, maps);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {

@@ -108,7 +108,8 @@ constexpr int kTBlock = GRPIC_TILED_BLOCK;
 
 // ---- shared-memory layout ----
 constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
-constexpr int kNodeStride = 8;                  // reals per node: D1 D2 D3 B1 B2 B3 + 2 pad (128-bit reads)
+// reals per node: D1 D2 D3 B1 B2 B3; FP32 pads to 8 (two 128-bit reads), FP64 keeps 6 (three 128-bit reads, 48 bytes)
+template <typename T> constexpr int kNodeStride = sizeof(T) == 4 ? 8 : 6;
 constexpr int kJStride = (kWinJ + 3) / 4 * 4;   // row stride of one shared J tile                  (24)
 constexpr int kJComp = kWinJ * kJStride;        // one component
 constexpr int kJTile = 3 * kJComp;              // one private J tile (J1 J2 J3)
@@ -117,13 +118,13 @@ constexpr int kRawComp = (kWinF * kRowF + 31) / 32 * 32;   // one staged compone
 constexpr int kRawElems = 6 * kRawComp;    // staged raw stencil; its space is reused by the J tiles after stage (i)
 constexpr int kJElems = kWarps * kJTile;        // one PRIVATE J tile per warp: no atomics inside the CTA
 constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
-constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride;
+template <typename T> constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride<T>;
 static_assert(kJTile % 4 == 0 && kFrontElems % 4 == 0, "128-bit zero fill");
 
 constexpr int kQueueVals = 8 * 64;            // reals per warp queue (8 x kQueue)
 template <typename T>
 constexpr size_t tiled_smem_bytes() {
-  return (size_t)(kFrontElems + kNodeElems + kWarps * kQueueVals) * sizeof(T) + (size_t)kWarps * 64 * sizeof(int) + 16;
+  return (size_t)(kFrontElems + kNodeElems<T> + kWarps * kQueueVals) * sizeof(T) + (size_t)kWarps * 64 * sizeof(int) + 16;
 }
 
 // offset inside a shared J tile of value q (0..7, layout of deposit_segments) relative to the cell's node
@@ -271,16 +272,16 @@ struct WarpQueue {
 // node-major shared field accessor: four node reads, six bilinear forms
 template <typename T>
 __device__ __forceinline__ void interp_nodes(const T* nod, int n00, T dx1, T dx2, T D[3], T B[3]) {
-  T c[4][kNodeStride];
+  T c[4][6];
   const int idx[4] = {n00, n00 + kNodeW, n00 + 1, n00 + kNodeW + 1};   // (0,0) (1,0) (0,1) (1,1)
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     if (sizeof(T) == 4) {
-      const float4* p = reinterpret_cast<const float4*>(nod + idx[k] * kNodeStride);
+      const float4* p = reinterpret_cast<const float4*>(nod + idx[k] * kNodeStride<T>);
       const float4 a = p[0], b = p[1];
       c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)a.z; c[k][3] = (T)a.w; c[k][4] = (T)b.x; c[k][5] = (T)b.y;
     } else {
-      const double2* p = reinterpret_cast<const double2*>(nod + idx[k] * kNodeStride);
+      const double2* p = reinterpret_cast<const double2*>(nod + idx[k] * kNodeStride<T>);
       const double2 a = p[0], b = p[1], d = p[2];
       c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)b.x; c[k][3] = (T)b.y; c[k][4] = (T)d.x; c[k][5] = (T)d.y;
     }
@@ -312,7 +313,7 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   extern __shared__ __align__(128) unsigned char smem_raw_[];
   T* sF = reinterpret_cast<T*>(smem_raw_);            // raw stencil, later the kWarps private J tiles
   T* sN = sF + kFrontElems;                           // node-major averaged fields
-  T* sQv = sN + kNodeElems;                           // per-warp straggler queues: values, then cells
+  T* sQv = sN + kNodeElems<T>;                           // per-warp straggler queues: values, then cells
   int* sQk = reinterpret_cast<int*>(sQv + kWarps * kQueueVals);
   uint64_t* bar = reinterpret_cast<uint64_t*>(sQk + kWarps * kQueue);
 
@@ -356,10 +357,10 @@ __global__ void __launch_bounds__(kTBlock, (sizeof(T) == 4 ? GRPIC_TILED_MINB : 
   for (int n = tid; n < kNodeW * kNodeW; n += kTBlock) {
     const int w1 = n / kNodeW, w2 = n % kNodeW;
     const RawAcc<T> acc{sF, w1 + 1, w2 + 1 + off2};
-    T* o = sN + n * kNodeStride;
+    T* o = sN + n * kNodeStride<T>;
 #pragma unroll
     for (int c = 0; c < 6; ++c) o[c] = node_value<T>(acc, c, yee_kind(c), 0, 0);
-    o[6] = T(0); o[7] = T(0);
+    if (kNodeStride<T> == 8) { o[6] = T(0); o[7] = T(0); }
   }
   __syncthreads();
   {                                                    // the raw stencil is dead: its space becomes the J tiles
