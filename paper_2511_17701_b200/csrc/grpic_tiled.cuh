@@ -109,7 +109,10 @@ constexpr int kTBlock = GRPIC_TILED_BLOCK;
 // ---- shared-memory layout ----
 constexpr int kNodeW = kWinC + 1;               // nodes per window edge: c .. c+1                  (23)
 // reals per node: D1 D2 D3 B1 B2 B3; FP32 pads to 8 (two 128-bit reads), FP64 keeps 6 (three 128-bit reads, 48 bytes)
-template <typename T> constexpr int kNodeStride = sizeof(T) == 4 ? 8 : 6;
+#ifndef GRPIC_NODE_STRIDE32
+#define GRPIC_NODE_STRIDE32 6
+#endif
+template <typename T> constexpr int kNodeStride = sizeof(T) == 4 ? GRPIC_NODE_STRIDE32 : 6;
 constexpr int kJStride = (kWinJ + 3) / 4 * 4;   // row stride of one shared J tile                  (24)
 constexpr int kJComp = kWinJ * kJStride;        // one component
 constexpr int kJTile = 3 * kJComp;              // one private J tile (J1 J2 J3)
@@ -118,7 +121,7 @@ constexpr int kRawComp = (kWinF * kRowF + 31) / 32 * 32;   // one staged compone
 constexpr int kRawElems = 6 * kRawComp;    // staged raw stencil; its space is reused by the J tiles after stage (i)
 constexpr int kJElems = kWarps * kJTile;        // one PRIVATE J tile per warp: no atomics inside the CTA
 constexpr int kFrontElems = kJElems > kRawElems ? kJElems : kRawElems;
-template <typename T> constexpr int kNodeElems = kNodeW * kNodeW * kNodeStride<T>;
+template <typename T> constexpr int kNodeElems = (kNodeW * kNodeW * kNodeStride<T> + 3) / 4 * 4;   // what follows stays 16-byte aligned
 static_assert(kJTile % 4 == 0 && kFrontElems % 4 == 0, "128-bit zero fill");
 
 constexpr int kQueueVals = 8 * 64;            // reals per warp queue (8 x kQueue)
@@ -276,10 +279,14 @@ __device__ __forceinline__ void interp_nodes(const T* nod, int n00, T dx1, T dx2
   const int idx[4] = {n00, n00 + kNodeW, n00 + 1, n00 + kNodeW + 1};   // (0,0) (1,0) (0,1) (1,1)
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    if (sizeof(T) == 4) {
+    if (sizeof(T) == 4 && kNodeStride<T> == 8) {
       const float4* p = reinterpret_cast<const float4*>(nod + idx[k] * kNodeStride<T>);
       const float4 a = p[0], b = p[1];
       c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)a.z; c[k][3] = (T)a.w; c[k][4] = (T)b.x; c[k][5] = (T)b.y;
+    } else if (sizeof(T) == 4) {
+      const float2* p = reinterpret_cast<const float2*>(nod + idx[k] * kNodeStride<T>);
+      const float2 a = p[0], b = p[1], d = p[2];
+      c[k][0] = (T)a.x; c[k][1] = (T)a.y; c[k][2] = (T)b.x; c[k][3] = (T)b.y; c[k][4] = (T)d.x; c[k][5] = (T)d.y;
     } else {
       const double2* p = reinterpret_cast<const double2*>(nod + idx[k] * kNodeStride<T>);
       const double2 a = p[0], b = p[1], d = p[2];
