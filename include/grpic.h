@@ -19,8 +19,12 @@
  *     exception and says so.  The structs themselves live in host memory and are read during the call.
  *   - The library owns only its context (constants, counters, sort scratch, tile table).
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default
- *     stream) and return without synchronising, except grpic_counters, grpic_sort (scratch allocation
- *     on first use and a 4-byte read-back of the alive count at its end) and grpic_step_host.
+ *     stream) and return without synchronising, except grpic_counters, grpic_updates_total, grpic_sorted_alive,
+ *     grpic_step_host, and the first grpic_sort of a context (scratch allocation).  grpic_step may use a side
+ *     stream of the context next to `cuda_stream`, forked from it and joined back into it with events: to the caller
+ *     everything is ordered on `cuda_stream`.
+ *   - A context belongs to the CUDA device that was current at grpic_create; calls made with another device
+ *     current return GRPIC_ESTATE.
  *   - Return value: GRPIC_OK (0) or a negative grpic_status; grpic_last_error(ctx) gives the text.
  *     Nothing aborts or throws.  There is no CPU fallback: without a CUDA device every compute
  *     call returns GRPIC_ECUDA.
@@ -104,8 +108,15 @@ int grpic_destroy(grpic_ctx* ctx);
  * "early_exit": 1 (default) leaves a fixed-point loop as soon as an iterate repeats the previous one bit
  *              for bit — every later iterate would be that same value, so the result IS the one of
  *              n_iter iterations; 0 always executes all n_iter (used by the test that proves this).
- * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernel after a grpic_sort;
+ * "tile_path": 1 (default) lets grpic_step use the shared-memory tile kernels after a grpic_sort;
  *              0 forces the direct kernel (global gathers and atomics).
+ * "lanes_path": 1 (default) sends the dense work items of a sorted species (at least "dense_min" particles of one
+ *              16 x 16-cell tile, default 2048, range 4..16384; read at the next grpic_sort) to k_step_lanes: one run of sorted
+ *              particles per lane, current accumulated in lane-private shared-memory windows, columns moved as 16-byte
+ *              blocks - this needs every particle column 16-byte aligned, otherwise (or with 0) all items stay with
+ *              the warp-by-warp tile kernel.  Same results up to the order of the J additions.
+ * "overlap":   1 (default) runs the small kernels of grpic_step (sparse items, slots behind the sorted range) on the side
+ *              stream beside k_step_lanes; 0 keeps everything on `cuda_stream`.
  * "tma": 1 (default) stages the tile's field stencil with TMA; 0 uses plain cooperative loads (also the
  *        automatic choice when a field array is not 16-byte aligned or (n2 + 2 nghost)*sizeof(real) % 16 != 0).
  * "host_chunk": particles per chunk of grpic_step_host, 2^10..2^26 (default 2^22; three chunks in flight). */
@@ -155,7 +166,9 @@ int grpic_step(grpic_ctx* ctx, grpic_particles* p, const grpic_fields* fields, g
  * of the present cell (i1, i2), or of the predicted cell when "sort_lookahead" > 0,
  * dead particles after all alive ones.  In place from the caller's view (library scratch inside).
  * Any order within one key is a correct result.  Builds the tile table that grpic_step's
- * shared-memory path uses for this species (keyed by the address of p->i1).
+ * shared-memory path uses for this species (keyed by the address of p->i1).  Enqueues and returns: the number of alive
+ * particles stays on the device (grpic_sorted_alive fetches it); only the first call on a context, or a call with more
+ * particles than any before, synchronises to (re)allocate scratch.
  * Errors: EINVAL, ENOMEM, ECUDA. */
 int grpic_sort(grpic_ctx* ctx, grpic_particles* p, void* cuda_stream);
 
@@ -169,7 +182,8 @@ int grpic_sort_into(grpic_ctx* ctx, const grpic_particles* src, grpic_particles*
 int grpic_tile_size(void);
 
 /* Compaction / injection support.  After grpic_sort the alive particles of the species occupy the slots
- * [0, n_alive) and the dead ones the rest; this call returns that n_alive (the caller may set p->n = n_alive to drop the
+ * [0, n_alive) and the dead ones the rest; this call returns that n_alive, read back from the device (it synchronises the
+ * stream of that sort, once per sort) (the caller may set p->n = n_alive to drop the
  * dead slots, or write new particles into slots >= n_alive with tag = 1, or append beyond p->n and raise p->n).
  * grpic_step pushes such slots through the direct kernel until the next grpic_sort, whatever was sorted before.
  * Errors: EINVAL, ESTATE (species never sorted on this context). */

@@ -8,6 +8,11 @@
 //                              shared memory by TMA, J in per-warp shared tiles, one flush (grpic_step; without the
 //                              deposit half: grpic_interp_push on a sorted species)
 //   k_deposit_tiled<T,C>       grpic_tiled.cuh: the deposit half alone               (grpic_deposit, sorted species)
+//   k_step_lanes<T,C>          grpic_lanes.cuh: the fused step over the DENSE work items of a sorted species — one run of
+//                              sorted particles per lane, lane-private J windows in shared memory, 128-bit column blocks
+//                              (grpic_step; k_step_tiled keeps the sparse items)
+//   k_push_or_step_from, k_deposit_from   the direct path over the slots behind the alive count of the last sort
+//   k_probe<kind>              grpic_probe.cuh: throughput probes (measured roofline denominators)
 //   k_sort_*, k_scan_*, k_items_*  counting sort by tile-major cell key + work-item table (grpic_sort)
 //   grpic_fields.cuh           field-solver half: auxiliary fields, Faraday, Ampere, boundary conditions, filter
 // C = coordinate class: Coord<T> (default map of the five configs, specialised) or CoordGen<T> (all maps of App. A).

@@ -5,16 +5,18 @@
 // has to find and resolve address conflicts between lanes in every iteration (match, butterfly, straggler queue):
 // 30 % of the instructions and almost half of the stall samples of a config-4 launch (profiles/r2_*).
 //
-// Here the item is cut the other way.  Every lane owns a CONTIGUOUS run of the item's particles
-// (count / kLThreads of them, in blocks of four), so the particles one lane sees one after the other are the
-// ones of one sorted cell, and lanes never work on neighbouring particles at the same time:
-//   - SoA columns move as 128-bit blocks (four particles of one column per lane): cp.async (LDGSTS.128) into a
-//     lane-private staging slot of shared memory, updated in place, written back with one LDS.128 + STG.128 per column;
+// Here the item is cut the other way, so that lanes never work on neighbouring particles at the same time:
+//   - the item's particles are cut into 16-byte blocks (four FP32 / two FP64 particles of one column); kLQuad consecutive
+//     lanes share a contiguous region and take its blocks in turn (whole 128-byte lines per warp instruction), each
+//     lane's own blocks staying within a region of about two sorted cells;
+//   - SoA columns move as 128-bit blocks: cp.async (LDGSTS.128) into a lane-private staging slot of shared memory,
+//     updated in place, written back with one LDS.128 + STG.128 per column;
 //   - J is accumulated in a lane-PRIVATE window of 3 x 3 cells (4 x 4 nodes x 3 components) in shared memory, laid out
-//     [slot][thread] so that a lane's window lives in the lane's own bank: plain conflict-free read-modify-writes,
+//     [slot][lane] so that a lane's window lives in the lane's own bank: plain conflict-free read-modify-writes,
 //     no atomics, no shuffles, no votes, no warp synchronisation anywhere in the particle loop;
-//   - a window is flushed to HBM/L2 with red.global.add when the run ends or moves far away; a path that leaves the
-//     window by a cell (drift since the sort) goes to L2 directly;
+//   - the window follows the SORTED cell of the lane's current block (offsets[] of the sort say where each key starts);
+//     nodes are addressed modulo 4, so a window that moves by a cell flushes (red.global.add) only the node column that
+//     leaves it; a path that leaves the window (drift since the sort) goes to L2 directly;
 //   - the field stencil of the tile is staged by TMA and averaged to nodes once per item, as in k_step_tiled.
 // The arithmetic of the path (grpic_device.cuh) is the same; only the order of the J additions differs.
 // Items too sparse for this to pay (less than `dense_min` particles: windows of one or two particles) stay with
