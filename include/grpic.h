@@ -189,6 +189,13 @@ int grpic_tile_size(void);
  * Errors: EINVAL, ESTATE (species never sorted on this context). */
 int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_alive);
 
+/* Drop the tile table the last grpic_sort built for this species (found by the address of p->i1): call it before the
+ * storage of a sorted species is freed or handed to another species, so that a recycled address cannot meet a stale
+ * table (results would still be right - every particle is tested against its tile's window - but the step would take the
+ * slow global path).  The library keeps at most 64 tables per context and evicts the one sorted longest ago.
+ * Synchronises the device (the table may still be in use).  Errors: EINVAL, ESTATE. */
+int grpic_forget(grpic_ctx* ctx, const grpic_particles* p);
+
 /* Counters of the most recent push/step (alive after it, absorbed inside, absorbed outside) and
  * of the most recent deposit/step (n_overstep).  Synchronises `cuda_stream`. Any pointer may be NULL. */
 int grpic_counters(grpic_ctx* ctx, int64_t* n_alive, int64_t* n_absorbed_in, int64_t* n_absorbed_out,

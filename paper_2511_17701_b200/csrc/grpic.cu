@@ -35,6 +35,7 @@ struct SortState {          // tile table of one species (keyed by the address o
   int64_t n_alive = 0;
   bool n_alive_known = false;
   cudaStream_t stream = nullptr;   // stream of the sort (the read-back waits on it)
+  uint64_t stamp = 0;              // ctx->stamp at the last sort: the oldest table goes when there are too many
   WorkItem* items = nullptr;
   uint32_t* d_n_items = nullptr;   // [0] items, [1] alive particles at sort time, [2] dense items
   uint32_t* dense_idx = nullptr;   // indices of the dense items (k_step_lanes), [max_items]
@@ -71,7 +72,8 @@ struct grpic_ctx {
   int64_t cap_particles;
   void* d_scratch;
   size_t scratch_bytes;
-  std::map<const void*, SortState> sorted;
+  std::map<const void*, SortState> sorted;   // at most kMaxTables entries (grpic_forget drops one; the oldest is evicted)
+  uint64_t stamp;
   // TMA
   TmaEncoder tma;
   // grpic_step_host buffers
@@ -306,6 +308,7 @@ int grpic_create(const grpic_grid* grid, double a, double r_min, double r_max, g
   ctx->d_counters = nullptr;
   ctx->d_keys = ctx->d_dest = ctx->d_hist = ctx->d_block_sums = ctx->d_tile_items = nullptr;
   ctx->cap_particles = 0;
+  ctx->stamp = 0;
   ctx->d_scratch = nullptr; ctx->scratch_bytes = 0;
   for (auto& q : ctx->h_dev) q = nullptr;
   ctx->f_scratch = nullptr; ctx->f_scratch_cells = 0;
@@ -655,8 +658,20 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* src, grpic_particles* p, cu
       sg, sp, n, src->i1, src->i2, src->tag, src->dx1, src->dx2, src->u1, src->u2, src->u3, ctx->d_keys, ctx->d_hist);
   if ((rc = scan_exclusive(ctx, ctx->d_hist, sg.n_keys + 1, st))) return rc;
 
-  // tile table from the offsets (before the cursor copy is consumed)
+  // tile table from the offsets (before the cursor copy is consumed).  Tables are keyed by the address of the i1
+  // column; a caller that keeps allocating new columns would grow the map without bound, so the table of the species
+  // sorted longest ago is dropped beyond kMaxTables (its next grpic_step simply takes the direct path).
+  constexpr size_t kMaxTables = 64;
+  if (ctx->sorted.find((const void*)p->i1) == ctx->sorted.end() && ctx->sorted.size() >= kMaxTables) {
+    auto oldest = ctx->sorted.begin();
+    for (auto it = ctx->sorted.begin(); it != ctx->sorted.end(); ++it)
+      if (it->second.stamp < oldest->second.stamp) oldest = it;
+    CK(cudaStreamSynchronize(st));
+    free_sort_state(oldest->second);                   // cudaFree waits for work that may still read the table
+    ctx->sorted.erase(oldest);
+  }
   SortState& ss = ctx->sorted[(const void*)p->i1];
+  ss.stamp = ++ctx->stamp;
   const uint32_t max_items = n_tiles + (uint32_t)((n + kChunk - 1) / kChunk);
   if (ss.max_items < max_items) {
     CK(cudaStreamSynchronize(st));
@@ -750,6 +765,16 @@ int grpic_sort_into(grpic_ctx* ctx, const grpic_particles* src, grpic_particles*
     for (int j = 0; j < 14; ++j)
       if (a[i] && a[i] == b[j]) return fail(ctx, GRPIC_EINVAL, "sort_into: src and dst share a column");
   return sort_impl(ctx, src, dst, (cudaStream_t)stream);
+}
+
+int grpic_forget(grpic_ctx* ctx, const grpic_particles* p) {
+  if (!ctx || !p) return fail(ctx, GRPIC_EINVAL, "NULL argument");
+  auto it = ctx->sorted.find((const void*)p->i1);
+  if (it == ctx->sorted.end()) return GRPIC_OK;
+  if (int rd = check_device(ctx)) return rd;
+  free_sort_state(it->second);                         // cudaFree waits for work that may still read the table
+  ctx->sorted.erase(it);
+  return GRPIC_OK;
 }
 
 int grpic_sorted_alive(grpic_ctx* ctx, const grpic_particles* p, int64_t* n_alive) {

@@ -24,7 +24,7 @@ EXPORTS = ["grpic_real_bytes", "grpic_create", "grpic_destroy", "grpic_set_int",
            "grpic_counters", "grpic_updates_total", "grpic_step_host", "grpic_last_error",
            "grpic_aux_fields", "grpic_faraday", "grpic_ampere", "grpic_fields_prepare", "grpic_fields_advance",
            "grpic_field_bc", "grpic_sorted_alive", "grpic_filter_current", "grpic_sort_into", "grpic_field_match",
-           "grpic_probe"]
+           "grpic_probe", "grpic_forget"]
 
 
 class GrpicError(RuntimeError):
@@ -98,6 +98,7 @@ def load(precision: str, build_if_missing: bool = False):
     lib.grpic_faraday.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_double, _vp]
     lib.grpic_ampere.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.POINTER(_Current), C.c_double, _vp]
     lib.grpic_sorted_alive.argtypes = [_vp, C.POINTER(_Particles), C.POINTER(C.c_int64)]
+    lib.grpic_forget.argtypes = [_vp, C.POINTER(_Particles)]
     lib.grpic_filter_current.argtypes = [_vp, C.POINTER(_Current), C.c_int32, _vp]
     lib.grpic_field_bc.argtypes = [_vp, C.POINTER(_Vec3), C.POINTER(_Vec3), C.c_int32, _vp]
     lib.grpic_field_match.argtypes = [_vp] + [C.POINTER(_Vec3)] * 4 + [C.c_double, _vp]
@@ -298,6 +299,11 @@ class Context:
         """out-of-place sort: src -> dst (two column sets that the caller swaps), no snapshot inside"""
         a = src.c_struct(); b = dst.c_struct()
         self._ck(self.lib.grpic_sort_into(self.h, C.byref(a), C.byref(b), _stream_ptr(stream)))
+
+    def forget(self, p: ParticleSet):
+        """drop the tile table of this species (before its storage is freed or reused)"""
+        ps = p.c_struct()
+        self._ck(self.lib.grpic_forget(self.h, C.byref(ps)))
 
     def sorted_alive(self, p: ParticleSet) -> int:
         """alive particles of the species at its last sort; they occupy the slots [0, n_alive)"""

@@ -903,6 +903,24 @@ def test_lanes_kernel_dense_and_degenerate_items(G, O, W, prec, dense_min, look)
         assert c["alive"] + c["absorbed_in"] + c["absorbed_out"] == n_alive
 
 
+def test_forget_drops_the_tile_table(G, O, W):
+    """grpic_forget: the table of a sorted species is gone (grpic_sorted_alive says so), and the species then steps
+    through the direct kernel with the same results."""
+    wl = W.config_magnetosphere(shrink=16)
+    g = grid_from_domain(O, wl.dom)
+    ctx = _ctx(G, wl.dom, "f32")
+    fdev, fhost = _fields_both(G, wl, "f32")
+    ps = G.ParticleSet.from_host(wl.species[0], "f32")
+    ctx.sort(ps)
+    assert ctx.sorted_alive(ps) == int(wl.species[0].tag.sum())
+    _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, "f32", "fused")
+    ctx.forget(ps)
+    with pytest.raises(G.GrpicError):
+        ctx.sorted_alive(ps)
+    _one_step_parity(G, O, ctx, g, ps, fdev, fhost, wl.dt, "f32", "fused")
+    ctx.forget(ps)                                     # nothing to forget: not an error
+
+
 def test_lanes_kernel_declines_unaligned_columns(G, O, W):
     """Columns that are only 4-byte aligned (views one element into a buffer): grpic_step must not take the 128-bit
     block path (include/grpic.h asks for 16-byte alignment; the library checks instead of trusting) and still be right."""
