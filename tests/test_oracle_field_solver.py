@@ -280,6 +280,8 @@ def test_absorbing_layer_fixed_point_edges_and_weight(O):
             s = (f[k][lay] - tgt[k][lay]) / (f0[k][lay] - tgt[k][lay])              # the weight actually applied
             assert np.allclose(s, s[:, :1], rtol=1e-9)                                # a function of r only
             assert np.all(np.diff(s[:, 0]) < 0) and 0.0 < s[-1, 0] and s[0, 0] < 1.0
+            # consistency with the profile reading R-F6 STATES (a re-statement: it pins nothing by itself; the behavioural
+            # assertions above and the pulse test below carry the layer, whose profile stays 'parity unpinned')
             assert np.allclose(s[:, 0], np.tanh(4 * (g.r_max - r[lay]) / (g.r_max - 9.0)), rtol=1e-9)
         # staggered components see a different radius than the node-centred ones in the same row
         row = np.nonzero((O.radius(g, np.arange(-G, g.n1 + G) + 0.0) > 9.0))[0][2]
